@@ -1,0 +1,153 @@
+"""CPU oracle for the Rosenbluth chain-generation hot path -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package. It is a ctypes front-end over
+``oracle/librosen_oracle.so`` (plain single-threaded C++, built by ``oracle/build.py``) and
+shares nothing with ``paper_1704_04381_b200`` -- neither imports the other.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+from .build import build as _build
+
+_LIB: Optional[C.CDLL] = None
+
+
+class _Summary(C.Structure):
+    _fields_ = [
+        ("n_chains", C.c_uint64), ("n_dead", C.c_uint64), ("n_steps_attempted", C.c_uint64),
+        ("ln_shift", C.c_double),
+        ("sum_w", C.c_double), ("sum_w_ree2", C.c_double), ("sum_w_rg2", C.c_double), ("sum_w2", C.c_double),
+        ("mean_ree2", C.c_double), ("mean_rg2", C.c_double), ("attrition", C.c_double), ("ln_mean_W", C.c_double),
+        ("digest_xor", C.c_uint64), ("digest_sum", C.c_uint64),
+    ]
+
+
+class _Outputs(C.Structure):
+    _fields_ = [
+        ("lnW", C.c_void_p), ("alive", C.c_void_p), ("m_seq", C.c_void_p), ("digest", C.c_void_p),
+        ("conf", C.c_void_p), ("ree2", C.c_void_p), ("rg2", C.c_void_p),
+    ]
+
+
+def lib() -> C.CDLL:
+    global _LIB
+    if _LIB is None:
+        path = _build()
+        L = C.CDLL(path)
+        L.oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
+        L.oracle_philox4x32_10.restype = None
+        L.oracle_lattice_free_dirs.argtypes = [C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32)]
+        L.oracle_lattice_free_dirs.restype = C.c_int32
+        L.oracle_direction.argtypes = [C.c_uint32, C.c_uint32, C.POINTER(C.c_float)]
+        L.oracle_direction.restype = None
+        L.oracle_lattice_generate.argtypes = [C.c_int32, C.c_uint64, C.c_uint64, C.c_uint64,
+                                              C.POINTER(_Outputs), C.POINTER(_Summary)]
+        L.oracle_lattice_generate.restype = C.c_int
+        L.oracle_realspace_generate.argtypes = [C.c_int32, C.c_uint64, C.c_int32, C.c_float, C.c_float,
+                                                C.c_uint64, C.c_uint64, C.POINTER(_Outputs), C.POINTER(_Summary)]
+        L.oracle_realspace_generate.restype = C.c_int
+        L.oracle_saw_enumerate.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
+                                           C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        L.oracle_saw_enumerate.restype = C.c_int
+        _LIB = L
+    return _LIB
+
+
+@dataclass
+class Result:
+    """Summary (dict of python scalars) and the requested per-chain numpy arrays."""
+    summary: dict
+    lnW: Optional[np.ndarray] = None
+    alive: Optional[np.ndarray] = None
+    m_seq: Optional[np.ndarray] = None
+    digest: Optional[np.ndarray] = None
+    conf: Optional[np.ndarray] = None
+    ree2: Optional[np.ndarray] = None
+    rg2: Optional[np.ndarray] = None
+
+
+def _alloc(n_chains: int, N: int, conf_dtype, want: set):
+    arrs = {}
+    if "lnW" in want: arrs["lnW"] = np.empty(n_chains, np.float64)
+    if "alive" in want: arrs["alive"] = np.empty(n_chains, np.uint8)
+    if "m_seq" in want: arrs["m_seq"] = np.empty((n_chains, N - 1), np.uint8)
+    if "digest" in want: arrs["digest"] = np.empty(n_chains, np.uint64)
+    if "conf" in want: arrs["conf"] = np.empty((n_chains, N, 3), conf_dtype)
+    if "ree2" in want: arrs["ree2"] = np.empty(n_chains, np.float64)
+    if "rg2" in want: arrs["rg2"] = np.empty(n_chains, np.float64)
+    out = _Outputs(*[arrs[k].ctypes.data if k in arrs else None
+                     for k in ("lnW", "alive", "m_seq", "digest", "conf", "ree2", "rg2")])
+    return arrs, out
+
+
+ALL = ("lnW", "alive", "m_seq", "digest", "conf", "ree2", "rg2")
+
+
+def _summary_dict(s: _Summary) -> dict:
+    return {name: getattr(s, name) for name, _ in _Summary._fields_}
+
+
+def lattice_generate(N: int, n_chains: int, seed: int, chain_offset: int = 0, outputs=ALL) -> Result:
+    arrs, out = _alloc(n_chains, N, np.int32, set(outputs))
+    s = _Summary()
+    rc = lib().oracle_lattice_generate(N, n_chains, seed, chain_offset, C.byref(out), C.byref(s))
+    if rc != 0:
+        raise ValueError(f"oracle_lattice_generate: invalid arguments (rc={rc})")
+    return Result(summary=_summary_dict(s), **arrs)
+
+
+def realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,
+                       chain_offset: int = 0, outputs=ALL) -> Result:
+    arrs, out = _alloc(n_chains, N, np.float32, set(outputs))
+    s = _Summary()
+    rc = lib().oracle_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset,
+                                         C.byref(out), C.byref(s))
+    if rc != 0:
+        raise ValueError(f"oracle_realspace_generate: invalid arguments (rc={rc})")
+    return Result(summary=_summary_dict(s), **arrs)
+
+
+def philox4x32_10(ctr, key) -> tuple:
+    c = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().oracle_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def lattice_free_dirs(r: np.ndarray) -> list:
+    """Free trial directions (indices into +x,-x,+y,-y,+z,-z) for the next monomer of walk r [s][3]."""
+    r = np.ascontiguousarray(r, dtype=np.int32)
+    fd = (C.c_int32 * 6)()
+    m = lib().oracle_lattice_free_dirs(r.ctypes.data_as(C.POINTER(C.c_int32)), r.shape[0], fd)
+    return [int(fd[i]) for i in range(m)]
+
+
+def direction(wz: int, wphi: int) -> np.ndarray:
+    u = (C.c_float * 3)()
+    lib().oracle_direction(wz & 0xFFFFFFFF, wphi & 0xFFFFFFFF, u)
+    return np.array([u[0], u[1], u[2]], dtype=np.float32)
+
+
+def saw_enumerate(n: int, fix_first: bool = False) -> dict:
+    """Brute-force enumeration of n-step cubic-lattice SAWs; see saw_enum.cpp.
+
+    Returns count, sum_ree2, sum_n2rg2 (integers, already multiplied by 6 when fix_first) and
+    ``hist``: dict {(a, b, c): number of walks with W = 2^a 3^b 5^c}.
+    """
+    hist = np.zeros((2 * n + 1, n + 1, n + 1), dtype=np.uint64)
+    cnt, s1, s2 = C.c_uint64(), C.c_uint64(), C.c_uint64()
+    rc = lib().oracle_saw_enumerate(n, int(fix_first), C.byref(cnt), C.byref(s1), C.byref(s2),
+                                    hist.ctypes.data_as(C.POINTER(C.c_uint64)))
+    if rc != 0:
+        raise RuntimeError(f"oracle_saw_enumerate rc={rc}")
+    mult = 6 if fix_first else 1
+    h = {tuple(int(i) for i in idx): int(hist[tuple(idx)]) * mult for idx in np.argwhere(hist)}
+    return {"count": cnt.value * mult, "sum_ree2": s1.value * mult, "sum_n2rg2": s2.value * mult, "hist": h}

@@ -1,0 +1,361 @@
+// rosen_oracle.cpp -- TEST INFRASTRUCTURE. Plain, slow, single-threaded CPU oracle for the
+// Rosenbluth chain-generation hot path of arXiv 1704.04381 (Guo & Baulin, CPC 2017).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// load this library. It shares no code, header, table or constant generator with the CUDA path
+// (paper_1704_04381_b200/csrc); both sides restate DESIGN.md section 3 ("numeric specification")
+// independently. Every function follows the paper's algorithm step by step, in its order and
+// notation; no blocking, fusion or pruning (the full j = 0..s-2 scans of Alg. 1 / Alg. 2 are kept).
+//
+// Citations are PAPER.md line numbers (= /root/reference/PAPER.md) plus section / algorithm.
+// Readings A1..A15 of the garbled / ambiguous passages are listed in DESIGN.md section 4.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"):
+//   philox4x32_10          : Random123 known-answer vectors (tests/golden/philox4x32_10_kat.txt)
+//   lattice free-site count: sum over ALL enumerated SAWs of 1/W == P_alive exactly (saw_enum.cpp)
+//   lattice grower+weights : mean(W) -> c_n, W-weighted <Ree2>,<Rg2> -> exact enumeration means
+//   real-space grower      : N=3 closed forms (free fraction 3/4, <Ree2>=2.5, <Rg2>=0.5),
+//                            sigma=0 freely-jointed chain (<Ree2>=(N-1)b^2, <Rg2>=b^2(N^2-1)/(6N))
+//   unit-sphere direction  : against fp64 libm cos/sin of the exact angle; |u|=1; moments
+//   parity unpinned        : none of the exported functions; real-space N>=4 with sigma>0 has no
+//                            closed form, it is covered by the invariants (bond length, no overlap)
+//                            and by the two special cases above only.
+//
+// Build: g++ -O2 -ffp-contract=off -shared -fPIC (see oracle/build.py). fp32 arithmetic of the
+// real-space path is written operation by operation with std::fmaf where DESIGN.md says "fma".
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------------
+// Result layouts (host memory; mirrors include/rosen.h field by field but is declared here
+// independently -- the oracle does not include the product header).
+// ---------------------------------------------------------------------------------------------
+struct oracle_summary {
+    uint64_t n_chains, n_dead, n_steps_attempted;
+    double   ln_shift;                                   // L
+    double   sum_w, sum_w_ree2, sum_w_rg2, sum_w2;       // w = exp(lnW - L); dead chains add 0
+    double   mean_ree2, mean_rg2, attrition, ln_mean_W;  // derived
+    uint64_t digest_xor, digest_sum;
+};
+
+struct oracle_outputs {     // every pointer optional (NULL = not written), HOST memory
+    double*   lnW;          // [n_chains]   -inf for dead chains
+    uint8_t*  alive;        // [n_chains]
+    uint8_t*  m_seq;        // [n_chains][N-1]  0 from the death step on
+    uint64_t* digest;       // [n_chains]
+    void*     conf;         // [n_chains][N][3] int32 (lattice) / float (real space); 0 after death
+    double*   ree2;         // [n_chains]
+    double*   rg2;          // [n_chains]
+};
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11). BASELINE north_star replaces the paper's
+// cuRAND generator (sec. 3.2) by this counter-based one; DESIGN.md 3.1.
+// ---------------------------------------------------------------------------------------------
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }   // Weyl key schedule
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n1 = (uint32_t)p1;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        const uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Word used by growth step s of chain `chain` for the uniform choice among free trials
+// (DESIGN.md 3.1 / reading A9): block counter (chain_lo, chain_hi, s>>2, 0), word s&3.
+static uint32_t selection_word(uint64_t seed, uint64_t chain, uint32_t s)
+{
+    const uint32_t ctr[4] = { (uint32_t)chain, (uint32_t)(chain >> 32), s >> 2, 0u };
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    return out[s & 3u];
+}
+
+// Per-chain digest of the decisions: FNV-1a style fold of one 32-bit token per
+// attempted step, token = m_s | choice_s << 8, choice = 0xFF on the death step.
+static inline uint64_t digest_init() { return 0xCBF29CE484222325ull; }
+static inline uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t choice)
+{
+    return (h ^ (uint64_t)(m | (choice << 8))) * 0x100000001B3ull;
+}
+
+// Neumaier compensated accumulator for the ensemble sums (so that the oracle's own rounding
+// does not eat the 1e-12 parity tolerance).
+struct Comp {
+    double s = 0.0, c = 0.0;
+    void add(double x) {
+        const double t = s + x;
+        if (std::fabs(s) >= std::fabs(x)) c += (s - t) + x; else c += (x - t) + s;
+        s = t;
+    }
+    double value() const { return s + c; }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Lattice: the six trial sites, in the fixed order +x,-x,+y,-y,+z,-z.
+// ---------------------------------------------------------------------------------------------
+static const int32_t E[6][3] = { {1,0,0}, {-1,0,0}, {0,1,0}, {0,-1,0}, {0,0,1}, {0,0,-1} };
+
+// Free-site list at a growth step (PAPER.md:126-149 Alg. 1 lines 9-23 overlap loop; :157-176
+// lines 24-34 neighbour count; readings A2, A3): trial d is free iff r[s-1]+e_d differs from
+// every earlier monomer r[j], j = 0..s-2 (the scan also covers j = s-1, which can never match).
+// r = s placed monomers [s][3]. Returns m = number of free trials, free_dirs[0..m) ascending.
+int32_t oracle_lattice_free_dirs(const int32_t* r, int32_t s, int32_t free_dirs[6])
+{
+    int32_t m = 0;
+    for (int d = 0; d < 6; ++d) {
+        const int32_t tx = r[3 * (s - 1) + 0] + E[d][0];
+        const int32_t ty = r[3 * (s - 1) + 1] + E[d][1];
+        const int32_t tz = r[3 * (s - 1) + 2] + E[d][2];
+        bool overlap = false;
+        for (int j = 0; j < s - 1; ++j)                                   // Alg. 1 line 13
+            if (r[3 * j] == tx && r[3 * j + 1] == ty && r[3 * j + 2] == tz) overlap = true;
+        if (!overlap) free_dirs[m++] = d;
+    }
+    return m;
+}
+
+static void finish_summary(oracle_summary* S, uint64_t n_chains, uint64_t n_dead, uint64_t n_steps,
+                           double L, const Comp& sw, const Comp& swr, const Comp& swg, const Comp& sw2,
+                           uint64_t dx, uint64_t ds)
+{
+    if (!S) return;
+    S->n_chains = n_chains; S->n_dead = n_dead; S->n_steps_attempted = n_steps; S->ln_shift = L;
+    S->sum_w = sw.value(); S->sum_w_ree2 = swr.value(); S->sum_w_rg2 = swg.value(); S->sum_w2 = sw2.value();
+    S->mean_ree2 = S->sum_w_ree2 / S->sum_w;                              // Eq. 2
+    S->mean_rg2  = S->sum_w_rg2 / S->sum_w;
+    S->attrition = (double)n_dead / (double)n_chains;
+    S->ln_mean_W = L + std::log(S->sum_w / (double)n_chains);             // Eq. 6
+    S->digest_xor = dx; S->digest_sum = ds;
+}
+
+// Cubic-lattice Rosenbluth generation, PAPER.md:100-179 (Alg. 1), Eq. 3 (:58), sec. 3.3.2.
+// Returns 0, or -1 on invalid arguments.
+int oracle_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                            const oracle_outputs* out, oracle_summary* summary)
+{
+    if (N < 2 || n_chains == 0) return -1;
+    const double L = std::log(6.0) + (double)(N - 2) * std::log(5.0);     // max possible lnW
+    std::vector<int32_t> r((size_t)N * 3);
+    Comp sw, swr, swg, sw2;
+    uint64_t n_dead = 0, n_steps = 0, dxor = 0, dsum = 0;
+
+    for (uint64_t i = 0; i < n_chains; ++i) {
+        const uint64_t chain = chain_offset + i;
+        std::fill(r.begin(), r.end(), 0);                                 // Pos[0] <- 0, :119
+        double lnW = 0.0;                                                 // W = 1
+        bool alive = true;
+        uint64_t h = digest_init();
+        uint8_t* mrow = (out && out->m_seq) ? out->m_seq + i * (size_t)(N - 1) : nullptr;
+        if (mrow) std::memset(mrow, 0, (size_t)(N - 1));
+
+        for (int32_t s = 1; s <= N - 1; ++s) {                            // Alg. 1 line 4
+            int32_t free_dirs[6];
+            const int32_t m = oracle_lattice_free_dirs(r.data(), s, free_dirs);
+            ++n_steps;
+            if (mrow) mrow[s - 1] = (uint8_t)m;
+            if (m == 0) {                                                 // dead end, :98; reading A6
+                alive = false; h = digest_fold(h, 0, 0xFF);
+                for (int32_t q = s; q < N; ++q) r[3*q] = r[3*q+1] = r[3*q+2] = 0;
+                break;
+            }
+            lnW += std::log((double)m);                                   // W *= 1/p_i = m, Eq. 3
+            const uint32_t u = selection_word(seed, chain, (uint32_t)s);
+            const uint32_t sel = (uint32_t)(((uint64_t)u * (uint64_t)m) >> 32);   // reading A7
+            const int32_t d = free_dirs[sel];
+            r[3*s+0] = r[3*(s-1)+0] + E[d][0];                            // Alg. 1 line 19
+            r[3*s+1] = r[3*(s-1)+1] + E[d][1];
+            r[3*s+2] = r[3*(s-1)+2] + E[d][2];
+            h = digest_fold(h, (uint32_t)m, (uint32_t)d);
+        }
+
+        // observables (sec. 4.1; Rg2 from north_star): integers until the divide
+        double ree2 = 0.0, rg2 = 0.0;
+        if (alive) {
+            int64_t sx = 0, sy = 0, sz = 0, s2 = 0;
+            for (int32_t q = 0; q < N; ++q) {
+                const int64_t x = r[3*q], y = r[3*q+1], z = r[3*q+2];
+                sx += x; sy += y; sz += z; s2 += x*x + y*y + z*z;
+            }
+            const int64_t ex = r[3*(N-1)] - r[0], ey = r[3*(N-1)+1] - r[1], ez = r[3*(N-1)+2] - r[2];
+            ree2 = (double)(ex*ex + ey*ey + ez*ez);
+            rg2  = (double)((int64_t)N * s2 - (sx*sx + sy*sy + sz*sz)) / ((double)N * (double)N);
+        } else {
+            lnW = -std::numeric_limits<double>::infinity(); ++n_dead;
+        }
+        const double w = alive ? std::exp(lnW - L) : 0.0;
+        sw.add(w); swr.add(w * ree2); swg.add(w * rg2); sw2.add(w * w);
+        dxor ^= h; dsum += h;
+
+        if (out) {
+            if (out->lnW) out->lnW[i] = lnW;
+            if (out->alive) out->alive[i] = alive ? 1 : 0;
+            if (out->digest) out->digest[i] = h;
+            if (out->ree2) out->ree2[i] = ree2;
+            if (out->rg2) out->rg2[i] = rg2;
+            if (out->conf) std::memcpy((int32_t*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(int32_t));
+        }
+    }
+    finish_summary(summary, n_chains, n_dead, n_steps, L, sw, swr, swg, sw2, dxor, dsum);
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Real space (PAPER.md:185-187 sec. 3.3.3, :202-262 Alg. 2).
+// ---------------------------------------------------------------------------------------------
+
+// "rngonsphere" (Alg. 2 line 10), re-specified on two Philox words so that it is
+// reproducible to the bit on any IEEE-754 machine (reading A10): only
+// + - * fma sqrt, all correctly rounded; no libm trigonometry.
+void oracle_direction(uint32_t wz, uint32_t wphi, float u[3])
+{
+    // z uniform on the 2^23 midpoints of (-1,1); exact in fp32
+    const float z = std::fmaf((float)(2u * (wz >> 9) + 1u), 0x1p-23f, -1.0f);
+    // azimuth: 24 bits = 3 octant bits + 21 fraction bits; odd octants are mirrored
+    const uint32_t a = wphi >> 8;
+    const uint32_t oct = a >> 21;
+    const uint32_t f = a & 0x1FFFFFu;
+    const uint32_t g = (oct & 1u) ? (0x1FFFFFu - f) : f;
+    const float x = (float)(2u * g + 1u) * 0x1.921fb6p-23f;             // (2g+1) * fl(pi/4 * 2^-22)
+    const float x2 = x * x;
+    // sin x, cos x on (0, pi/4): Taylor polynomials, coefficients = fp32-nearest of +-1/n!
+    float p = std::fmaf(x2, 0x1.71de3ap-19f, -0x1.a01a02p-13f);          // 1/9!, -1/7!
+    p = std::fmaf(x2, p, 0x1.111112p-7f);                                // 1/5!
+    p = std::fmaf(x2, p, -0x1.555556p-3f);                               // -1/3!
+    p = p * x2;
+    const float sn = std::fmaf(x, p, x);
+    float q = std::fmaf(x2, -0x1.27e4fcp-22f, 0x1.a01a02p-16f);          // -1/10!, 1/8!
+    q = std::fmaf(x2, q, -0x1.6c16c2p-10f);                              // -1/6!
+    q = std::fmaf(x2, q, 0x1.555556p-5f);                                // 1/4!
+    q = std::fmaf(x2, q, -0.5f);                                         // -1/2!
+    const float cs = std::fmaf(x2, q, 1.0f);
+    // octant table (cos phi, sin phi): 0:(c,s) 1:(s,c) 2:(-s,c) 3:(-c,s) 4:(-c,-s) 5:(-s,-c) 6:(s,-c) 7:(c,-s)
+    const bool swap = (((oct + 1u) >> 1) & 1u) != 0;
+    float cx = swap ? sn : cs;
+    float sy = swap ? cs : sn;
+    if (oct >= 2u && oct <= 5u) cx = -cx;
+    if (oct >= 4u) sy = -sy;
+    const float rho = std::sqrt(std::fmaf(-z, z, 1.0f));
+    u[0] = rho * cx; u[1] = rho * sy; u[2] = z;
+}
+
+// Words of trial t at growth step s (DESIGN.md 3.1 / reading A9): block counter
+// (chain_lo, chain_hi, s, 1 + (t>>1)); even t takes words (0,1), odd t words (2,3).
+static void trial_words(uint64_t seed, uint64_t chain, uint32_t s, uint32_t t, uint32_t* wz, uint32_t* wphi)
+{
+    const uint32_t ctr[4] = { (uint32_t)chain, (uint32_t)(chain >> 32), s, 1u + (t >> 1) };
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    *wz = out[2 * (t & 1u)]; *wphi = out[2 * (t & 1u) + 1];
+}
+
+int oracle_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                              uint64_t seed, uint64_t chain_offset,
+                              const oracle_outputs* out, oracle_summary* summary)
+{
+    if (N < 2 || n_chains == 0 || k_trials < 1 || k_trials > 255) return -1;
+    if (!(bond_len > 0.0f) || !(sigma >= 0.0f) || !std::isfinite(bond_len) || !std::isfinite(sigma)) return -1;
+    const int32_t k = k_trials;
+    const float b = bond_len;
+    const float sigma2 = sigma * sigma;                                   // rounded once to fp32
+    const double L = (double)(N - 1) * std::log((double)k);
+    std::vector<float> r((size_t)N * 3);
+    std::vector<float> trial((size_t)k * 3);
+    std::vector<int32_t> free_t((size_t)k);
+    Comp sw, swr, swg, sw2;
+    uint64_t n_dead = 0, n_steps = 0, dxor = 0, dsum = 0;
+
+    for (uint64_t i = 0; i < n_chains; ++i) {
+        const uint64_t chain = chain_offset + i;
+        std::fill(r.begin(), r.end(), 0.0f);                              // Pos[0] <- 0, :216
+        double lnW = 0.0;
+        bool alive = true;
+        uint64_t h = digest_init();
+        uint8_t* mrow = (out && out->m_seq) ? out->m_seq + i * (size_t)(N - 1) : nullptr;
+        if (mrow) std::memset(mrow, 0, (size_t)(N - 1));
+
+        for (int32_t s = 1; s <= N - 1; ++s) {                            // Alg. 2 line 4
+            const float hx = r[3*(s-1)], hy = r[3*(s-1)+1], hz = r[3*(s-1)+2];
+            int32_t m = 0;
+            for (int32_t t = 0; t < k; ++t) {                             // Alg. 2 line 9, ptMax = k
+                uint32_t wz, wphi; float u[3];
+                trial_words(seed, chain, (uint32_t)s, (uint32_t)t, &wz, &wphi);
+                oracle_direction(wz, wphi, u);                            // rngonsphere, line 10
+                const float tx = std::fmaf(b, u[0], hx);                  // line 11
+                const float ty = std::fmaf(b, u[1], hy);
+                const float tz = std::fmaf(b, u[2], hz);
+                trial[3*t] = tx; trial[3*t+1] = ty; trial[3*t+2] = tz;
+                bool overlap = false;
+                for (int32_t j = 0; j < s - 1; ++j) {                     // line 13, half-open (A2)
+                    const float dx = r[3*j] - tx, dy = r[3*j+1] - ty, dz = r[3*j+2] - tz;
+                    const float d2 = std::fmaf(dz, dz, std::fmaf(dy, dy, dx * dx));   // "distance", :235
+                    if (d2 < sigma2) overlap = true;                      // strict <, sigma (A11)
+                }
+                if (!overlap) free_t[m++] = t;                            // counts TRIALS (A5)
+            }
+            ++n_steps;
+            if (mrow) mrow[s - 1] = (uint8_t)m;
+            if (m == 0) {                                                 // N_allowed = 0, :187; A6
+                alive = false; h = digest_fold(h, 0, 0xFF);
+                for (int32_t q = s; q < N; ++q) r[3*q] = r[3*q+1] = r[3*q+2] = 0.0f;
+                break;
+            }
+            lnW += std::log((double)m);                                   // W *= N_allowed (A4)
+            const uint32_t u32 = selection_word(seed, chain, (uint32_t)s);
+            const uint32_t sel = (uint32_t)(((uint64_t)u32 * (uint64_t)m) >> 32);
+            const int32_t t = free_t[sel];
+            r[3*s] = trial[3*t]; r[3*s+1] = trial[3*t+1]; r[3*s+2] = trial[3*t+2];   // line 21
+            h = digest_fold(h, (uint32_t)m, (uint32_t)t);
+        }
+
+        double ree2 = 0.0, rg2 = 0.0;
+        if (alive) {
+            double cx = 0.0, cy = 0.0, cz = 0.0;
+            for (int32_t q = 0; q < N; ++q) { cx += (double)r[3*q]; cy += (double)r[3*q+1]; cz += (double)r[3*q+2]; }
+            cx /= (double)N; cy /= (double)N; cz /= (double)N;
+            double acc = 0.0;
+            for (int32_t q = 0; q < N; ++q) {
+                const double ax = (double)r[3*q] - cx, ay = (double)r[3*q+1] - cy, az = (double)r[3*q+2] - cz;
+                acc += ax*ax + ay*ay + az*az;
+            }
+            rg2 = acc / (double)N;
+            const double ex = (double)r[3*(N-1)] - (double)r[0], ey = (double)r[3*(N-1)+1] - (double)r[1],
+                         ez = (double)r[3*(N-1)+2] - (double)r[2];
+            ree2 = ex*ex + ey*ey + ez*ez;
+        } else {
+            lnW = -std::numeric_limits<double>::infinity(); ++n_dead;
+        }
+        const double w = alive ? std::exp(lnW - L) : 0.0;
+        sw.add(w); swr.add(w * ree2); swg.add(w * rg2); sw2.add(w * w);
+        dxor ^= h; dsum += h;
+
+        if (out) {
+            if (out->lnW) out->lnW[i] = lnW;
+            if (out->alive) out->alive[i] = alive ? 1 : 0;
+            if (out->digest) out->digest[i] = h;
+            if (out->ree2) out->ree2[i] = ree2;
+            if (out->rg2) out->rg2[i] = rg2;
+            if (out->conf) std::memcpy((float*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(float));
+        }
+    }
+    finish_summary(summary, n_chains, n_dead, n_steps, L, sw, swr, swg, sw2, dxor, dsum);
+    return 0;
+}
+
+}  // extern "C"
