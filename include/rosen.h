@@ -1,0 +1,152 @@
+/*
+ * rosen.h -- C ABI of librosen.so: Rosenbluth self-avoiding-walk chain generation on one B200.
+ *
+ * The data-parallel hot path of arXiv 1704.04381 (Guo & Baulin, "GPU Implementation of the
+ * Rosenbluth Generation Method for Static Monte Carlo Simulations", CPC 2017), re-designed for
+ * sm_100a. Citations are /root/reference/PAPER.md line numbers; the numeric specification both
+ * this library and the CPU oracle restate independently is DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every entry point returns ROSEN_OK (0) or a negative ROSEN_E* code; nothing throws.
+ *   - All pointers inside rosen_outputs point to CALLER-OWNED memory; `memory` says whether they
+ *     are device pointers (ROSEN_MEM_DEVICE, the usual case: PyTorch tensors) or host pointers
+ *     (ROSEN_MEM_HOST: the library stages through its own device buffers and copies back inside
+ *     the call). NULL members are not written. The library allocates nothing the caller must free.
+ *   - `summary` is always a HOST pointer (may be NULL). When it is non-NULL the call returns after
+ *     the work has completed on `cuda_stream` (the stream is synchronised); when it is NULL and
+ *     all outputs are device memory the call only enqueues work on `cuda_stream`.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Chain ids: chain i of a call has id chain_offset + i. Every per-chain result is a pure
+ *     function of (seed, id, parameters): any sub-range reproduces bit-identically, which is how
+ *     multi-GPU sharding, resume and sampled parity checks work.
+ *   - There is no CPU fallback: without a CUDA device every generate call fails with ROSEN_ECUDA.
+ */
+#ifndef ROSEN_H
+#define ROSEN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define ROSEN_API __attribute__((visibility("default")))
+#else
+#define ROSEN_API
+#endif
+
+#define ROSEN_OK        0
+#define ROSEN_EINVAL   (-1)  /* N < 2, n_chains == 0, k_trials outside 1..255, bond_len <= 0, sigma < 0, NaN/inf */
+#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 512, real space 1024)             */
+#define ROSEN_ECUDA    (-3)  /* a CUDA runtime call failed (no device, launch error, ...); see rosen_last_error */
+#define ROSEN_ENOMEM   (-4)  /* staging / workspace allocation failed                                           */
+
+#define ROSEN_MEM_DEVICE 0
+#define ROSEN_MEM_HOST   1
+
+#define ROSEN_LATTICE_MAX_N    512
+#define ROSEN_REALSPACE_MAX_N 1024
+
+/*
+ * Ensemble summary, Eq. 2 and Eq. 6 (:362). w_c = exp(lnW_c - ln_shift) for a chain
+ * that reached N monomers and 0 for a dead chain; dead chains stay in every denominator
+ * (reading A6 in DESIGN.md 4). All sums are deterministic: fixed chain->thread->block mapping,
+ * warp shuffle tree, block tree, then a second kernel over the block partials; no float atomics.
+ */
+typedef struct rosen_summary {
+    uint64_t n_chains;            /* chains attempted                                                  */
+    uint64_t n_dead;              /* chains that hit m_s = 0                                           */
+    uint64_t n_steps_attempted;   /* sum over chains of growth steps attempted (= monomer-steps)       */
+    double   ln_shift;            /* L: lattice ln6 + (N-2) ln5, real space (N-1) ln k                 */
+    double   sum_w, sum_w_ree2, sum_w_rg2, sum_w2;
+    double   mean_ree2;           /* sum_w_ree2 / sum_w   : W-weighted <R_ee^2>                        */
+    double   mean_rg2;            /* sum_w_rg2 / sum_w    : W-weighted <R_g^2>                         */
+    double   attrition;           /* n_dead / n_chains                                                 */
+    double   ln_mean_W;           /* L + ln(sum_w / n_chains) = ln Z_N estimate (Eq. 6)                */
+    uint64_t digest_xor;          /* XOR / wrapping sum of the per-chain digests; 0 unless             */
+    uint64_t digest_sum;          /*   outputs->digest was requested                                   */
+} rosen_summary;
+
+/*
+ * Optional per-chain outputs ("coordinates of each conformation and corresponding Rosenbluth
+ * weight are flushed to the global memory"). Layouts are chain-major, C order.
+ */
+typedef struct rosen_outputs {
+    double*   lnW;     /* [n_chains]            ln W = sum_s ln m_s (Eq. 3, :58); -inf for dead chains        */
+    uint8_t*  alive;   /* [n_chains]            1 = reached N monomers                                         */
+    uint8_t*  m_seq;   /* [n_chains][N-1]       m_s = number of free trials at step s; 0 from death on         */
+    uint64_t* digest;  /* [n_chains]            FNV-1a fold of (m_s | choice_s << 8) per attempted step        */
+    void*     conf;    /* [n_chains][N][3]      int32 (lattice) / float (real space); 0 after the death step   */
+    double*   ree2;    /* [n_chains]            |r_{N-1} - r_0|^2; 0 for dead chains                           */
+    double*   rg2;     /* [n_chains]            (1/N) sum_i |r_i - r_cm|^2; 0 for dead chains                  */
+    int32_t   memory;  /* ROSEN_MEM_DEVICE or ROSEN_MEM_HOST for ALL pointers above                            */
+    int32_t   reserved;
+} rosen_outputs;
+
+/*
+ * Cubic-lattice Rosenbluth generation (sec. 3.3.2 + Algorithm 1; weight Eq. 3).
+ * Each chain starts at the origin and grows to N monomers; at step s (1..N-1) the 6 neighbours of
+ * r_{s-1}, in the order +x,-x,+y,-y,+z,-z, are tested against all earlier monomers, m_s = number
+ * of free ones, lnW += ln m_s, and the ((u_s * m_s) >> 32)-th free neighbour is taken, u_s being
+ * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
+ * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N.
+ */
+ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                           const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
+
+/*
+ * Real-space (off-lattice) Rosenbluth generation (PAPER.md:185-187 sec. 3.3.3, :202-262 Alg. 2).
+ * At step s, k_trials unit directions u_t come from Philox blocks (id_lo, id_hi, s, 1 + (t>>1))
+ * (words 0,1 for even t, 2,3 for odd t) through the fp32 map of DESIGN.md 3.3; trial_t =
+ * fma(bond_len, u_t, r_{s-1}); it overlaps if fma(dz,dz,fma(dy,dy,dx*dx)) < sigma*sigma (fp32)
+ * for some j <= s-2; m_s = number of non-overlapping trials; the ((u_s*m_s)>>32)-th of them in
+ * trial order is taken, u_s as in the lattice call. 2 <= N <= ROSEN_REALSPACE_MAX_N,
+ * 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, both finite.
+ */
+ROSEN_API int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                             uint64_t seed, uint64_t chain_offset,
+                             const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
+
+/*
+ * Conformation dump alone (the store path of PAPER.md:80 / :189, BASELINE config 5): identical to
+ * the generate calls with outputs = {conf, lnW} only, provided as named entry points.
+ * conf/lnW are DEVICE pointers when memory == ROSEN_MEM_DEVICE, host pointers otherwise.
+ */
+ROSEN_API int rosen_lattice_dump(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                       int32_t* conf, double* lnW, int32_t memory, rosen_summary* summary, void* cuda_stream);
+ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                         uint64_t seed, uint64_t chain_offset,
+                         float* conf, double* lnW, int32_t memory, rosen_summary* summary, void* cuda_stream);
+
+/*
+ * Merge the summaries of disjoint chain ranges generated with the same (N, k_trials) -- the only
+ * "exchange" a multi-GPU run needs. Sums are added in array order (deterministic),
+ * derived fields recomputed. Returns ROSEN_EINVAL if count == 0 or the ln_shift values differ.
+ * Pure host function.
+ */
+ROSEN_API int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged);
+
+/* Bytes of device scratch the library keeps per device for block partials (informational). */
+ROSEN_API size_t rosen_workspace_bytes(void);
+
+/*
+ * Number of kernel launches the last generate/dump call on this thread enqueued, and the name of
+ * the main kernel variant it chose (static string). For bench.py's gpu_launches and profiles.
+ */
+ROSEN_API int32_t     rosen_last_launch_count(void);
+ROSEN_API const char* rosen_last_kernel_name(void);
+
+/* Static description of an error code; rosen_last_error() adds the CUDA error text of the last
+ * failing call on this thread (empty string if none). */
+ROSEN_API const char* rosen_strerror(int code);
+ROSEN_API const char* rosen_last_error(void);
+
+/* Library version string, e.g. "rosen-b200 0.1 (sm_100a)". */
+ROSEN_API const char* rosen_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ROSEN_H */

@@ -1,0 +1,219 @@
+"""Thin Python binding of the C ABI in include/rosen.h (argument marshalling only).
+
+Same names as the C entry points. PyTorch is used for device memory (output tensors) and for the
+current CUDA stream; every step of the path runs inside librosen.so's kernels. There is no CPU
+fallback: if the library is missing or no CUDA device is present the calls raise RosenError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Iterable, Optional, Tuple
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librosen.so")
+
+ROSEN_OK, ROSEN_EINVAL, ROSEN_ERANGE, ROSEN_ECUDA, ROSEN_ENOMEM = 0, -1, -2, -3, -4
+ROSEN_MEM_DEVICE, ROSEN_MEM_HOST = 0, 1
+
+PER_CHAIN = ("lnW", "alive", "m_seq", "digest", "conf", "ree2", "rg2")
+
+
+class RosenError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"librosen error {code}: {message}")
+        self.code = code
+
+
+class rosen_summary(C.Structure):
+    _fields_ = [
+        ("n_chains", C.c_uint64), ("n_dead", C.c_uint64), ("n_steps_attempted", C.c_uint64),
+        ("ln_shift", C.c_double),
+        ("sum_w", C.c_double), ("sum_w_ree2", C.c_double), ("sum_w_rg2", C.c_double), ("sum_w2", C.c_double),
+        ("mean_ree2", C.c_double), ("mean_rg2", C.c_double), ("attrition", C.c_double), ("ln_mean_W", C.c_double),
+        ("digest_xor", C.c_uint64), ("digest_sum", C.c_uint64),
+    ]
+
+    def as_dict(self) -> Dict[str, float]:
+        return {name: getattr(self, name) for name, _ in self._fields_}
+
+    @classmethod
+    def from_dict(cls, d: Dict[str, float]) -> "rosen_summary":
+        return cls(**{name: d[name] for name, _ in cls._fields_})
+
+
+class rosen_outputs(C.Structure):
+    _fields_ = [
+        ("lnW", C.c_void_p), ("alive", C.c_void_p), ("m_seq", C.c_void_p), ("digest", C.c_void_p),
+        ("conf", C.c_void_p), ("ree2", C.c_void_p), ("rg2", C.c_void_p),
+        ("memory", C.c_int32), ("reserved", C.c_int32),
+    ]
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen librosen.so and declare every symbol of include/rosen.h. Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RosenError(ROSEN_ECUDA, f"{LIB_PATH} not built -- run `python -m paper_1704_04381_b200.build` "
+                                      "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    u64, i32, vp = C.c_uint64, C.c_int32, C.c_void_p
+    L.rosen_lattice_generate.argtypes = [i32, u64, u64, u64, C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
+    L.rosen_lattice_generate.restype = C.c_int
+    L.rosen_realspace_generate.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64,
+                                           C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
+    L.rosen_realspace_generate.restype = C.c_int
+    L.rosen_lattice_dump.argtypes = [i32, u64, u64, u64, vp, vp, i32, C.POINTER(rosen_summary), vp]
+    L.rosen_lattice_dump.restype = C.c_int
+    L.rosen_realspace_dump.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64, vp, vp, i32,
+                                       C.POINTER(rosen_summary), vp]
+    L.rosen_realspace_dump.restype = C.c_int
+    L.rosen_summary_merge.argtypes = [C.POINTER(rosen_summary), i32, C.POINTER(rosen_summary)]
+    L.rosen_summary_merge.restype = C.c_int
+    L.rosen_workspace_bytes.argtypes = []
+    L.rosen_workspace_bytes.restype = C.c_size_t
+    L.rosen_last_launch_count.argtypes = []
+    L.rosen_last_launch_count.restype = i32
+    for name in ("rosen_last_kernel_name", "rosen_last_error", "rosen_version"):
+        getattr(L, name).argtypes = []
+        getattr(L, name).restype = C.c_char_p
+    L.rosen_strerror.argtypes = [C.c_int]
+    L.rosen_strerror.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> None:
+    if rc != ROSEN_OK:
+        L = load_library()
+        detail = L.rosen_last_error().decode()
+        raise RosenError(rc, L.rosen_strerror(rc).decode() + (f" ({detail})" if detail else ""))
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _alloc_outputs(N: int, n_chains: int, conf_dtype: str, outputs: Iterable[str], device, host: bool):
+    """Allocate the requested per-chain buffers: torch CUDA tensors, or pinned host tensors."""
+    torch = _torch()
+    want = set(outputs)
+    unknown = want - set(PER_CHAIN)
+    if unknown:
+        raise ValueError(f"unknown outputs {sorted(unknown)}; choose from {PER_CHAIN}")
+    kw = dict(device="cpu", pin_memory=True) if host else dict(device=device)
+    shapes = {
+        "lnW": ((n_chains,), torch.float64), "alive": ((n_chains,), torch.uint8),
+        "m_seq": ((n_chains, N - 1), torch.uint8), "digest": ((n_chains,), torch.int64),
+        "conf": ((n_chains, N, 3), torch.int32 if conf_dtype == "int32" else torch.float32),
+        "ree2": ((n_chains,), torch.float64), "rg2": ((n_chains,), torch.float64),
+    }
+    tensors = {k: torch.empty(shapes[k][0], dtype=shapes[k][1], **kw) for k in PER_CHAIN if k in want}
+    st = rosen_outputs(*[tensors[k].data_ptr() if k in tensors else None for k in PER_CHAIN],
+                       ROSEN_MEM_HOST if host else ROSEN_MEM_DEVICE, 0)
+    return tensors, st
+
+
+def _stream_ptr(stream) -> int:
+    torch = _torch()
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def rosen_lattice_generate(N: int, n_chains: int, seed: int, chain_offset: int = 0, outputs: Iterable[str] = (),
+                           summary: bool = True, stream=None, host_outputs: bool = False, device=None
+                           ) -> Tuple[Optional[Dict[str, float]], Dict[str, "object"]]:
+    """rosen_lattice_generate of include/rosen.h. Returns (summary dict or None, {name: tensor})."""
+    L = load_library()
+    torch = _torch()
+    device = device if device is not None else torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
+    if device is None:
+        raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
+    tensors, st = _alloc_outputs(N, n_chains, "int32", outputs, device, host_outputs)
+    s = rosen_summary()
+    _check(L.rosen_lattice_generate(N, n_chains, seed, chain_offset, C.byref(st),
+                                    C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), tensors
+
+
+def rosen_realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,
+                             chain_offset: int = 0, outputs: Iterable[str] = (), summary: bool = True, stream=None,
+                             host_outputs: bool = False, device=None
+                             ) -> Tuple[Optional[Dict[str, float]], Dict[str, "object"]]:
+    """rosen_realspace_generate of include/rosen.h. Returns (summary dict or None, {name: tensor})."""
+    L = load_library()
+    torch = _torch()
+    device = device if device is not None else torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
+    if device is None:
+        raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
+    tensors, st = _alloc_outputs(N, n_chains, "float32", outputs, device, host_outputs)
+    s = rosen_summary()
+    _check(L.rosen_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, C.byref(st),
+                                      C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), tensors
+
+
+def rosen_lattice_dump(N: int, n_chains: int, seed: int, chain_offset: int = 0, conf=None, lnW=None,
+                       summary: bool = True, stream=None):
+    """rosen_lattice_dump: conf int32 [n_chains, N, 3] and lnW float64 [n_chains] CUDA tensors (allocated if None)."""
+    L = load_library()
+    torch = _torch()
+    conf = conf if conf is not None else torch.empty((n_chains, N, 3), dtype=torch.int32, device="cuda")
+    lnW = lnW if lnW is not None else torch.empty((n_chains,), dtype=torch.float64, device="cuda")
+    s = rosen_summary()
+    _check(L.rosen_lattice_dump(N, n_chains, seed, chain_offset, conf.data_ptr(), lnW.data_ptr(), ROSEN_MEM_DEVICE,
+                                C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), conf, lnW
+
+
+def rosen_realspace_dump(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,
+                         chain_offset: int = 0, conf=None, lnW=None, summary: bool = True, stream=None):
+    """rosen_realspace_dump: conf float32 [n_chains, N, 3] and lnW float64 [n_chains] CUDA tensors."""
+    L = load_library()
+    torch = _torch()
+    conf = conf if conf is not None else torch.empty((n_chains, N, 3), dtype=torch.float32, device="cuda")
+    lnW = lnW if lnW is not None else torch.empty((n_chains,), dtype=torch.float64, device="cuda")
+    s = rosen_summary()
+    _check(L.rosen_realspace_dump(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, conf.data_ptr(),
+                                  lnW.data_ptr(), ROSEN_MEM_DEVICE, C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), conf, lnW
+
+
+def rosen_summary_merge(parts) -> Dict[str, float]:
+    """rosen_summary_merge: merge summary dicts of disjoint chain ranges (rank order)."""
+    L = load_library()
+    arr = (rosen_summary * len(parts))(*[rosen_summary.from_dict(p) for p in parts])
+    out = rosen_summary()
+    _check(L.rosen_summary_merge(arr, len(parts), C.byref(out)))
+    return out.as_dict()
+
+
+def rosen_workspace_bytes() -> int:
+    return int(load_library().rosen_workspace_bytes())
+
+
+def rosen_last_launch_count() -> int:
+    return int(load_library().rosen_last_launch_count())
+
+
+def rosen_last_kernel_name() -> str:
+    return load_library().rosen_last_kernel_name().decode()
+
+
+def rosen_strerror(code: int) -> str:
+    return load_library().rosen_strerror(code).decode()
+
+
+def rosen_last_error() -> str:
+    return load_library().rosen_last_error().decode()
+
+
+def rosen_version() -> str:
+    return load_library().rosen_version().decode()

@@ -1,0 +1,270 @@
+// api.cu -- the C ABI of librosen.so (include/rosen.h): argument validation, per-device scratch,
+// host-pointer staging, launches, summary assembly. No compute happens on the host: every step of
+// the path runs in the kernels of lattice.cu / realspace.cu / reduce.cu.
+#include "../../include/rosen.h"
+#include "common.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+namespace {
+
+using rosen::DevOutputs;
+using rosen::Partial;
+
+thread_local char g_err[512] = "";
+thread_local int32_t g_launches = 0;
+thread_local const char* g_kernel = "";
+
+int fail_cuda(cudaError_t e, const char* what)
+{
+    std::snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    cudaGetLastError();   // clear the sticky-less error state
+    return ROSEN_ECUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(e_, #call); } while (0)
+
+// Per-device scratch: block partials + one total, and a pinned host mirror of the total.
+struct Scratch {
+    Partial* dev = nullptr;       // [kMaxPartials + 1]
+    Partial* host = nullptr;      // pinned, 1 element
+};
+constexpr int kMaxDevices = 64;
+Scratch g_scratch[kMaxDevices];
+std::mutex g_mutex;
+
+int get_scratch(Scratch** out)
+{
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) { std::snprintf(g_err, sizeof(g_err), "device index %d unsupported", dev); return ROSEN_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_mutex);
+    Scratch& s = g_scratch[dev];
+    if (!s.dev) {
+        CK(cudaMalloc(&s.dev, sizeof(Partial) * (rosen::kMaxPartials + 1)));
+        CK(cudaMallocHost(&s.host, sizeof(Partial)));
+    }
+    *out = &s;
+    return ROSEN_OK;
+}
+
+struct Sizes { size_t lnW, alive, m_seq, digest, conf, ree2, rg2; };
+
+Sizes output_sizes(int32_t N, uint64_t n, size_t conf_elem)
+{
+    Sizes z;
+    z.lnW = n * sizeof(double); z.alive = n; z.m_seq = n * (size_t)(N - 1); z.digest = n * sizeof(uint64_t);
+    z.conf = n * (size_t)N * 3 * conf_elem; z.ree2 = n * sizeof(double); z.rg2 = n * sizeof(double);
+    return z;
+}
+
+// Staging of HOST output pointers: device twins allocated on the stream, copied back, freed.
+struct Staging {
+    DevOutputs dev{};
+    bool staged = false;
+    cudaStream_t stream = nullptr;
+    ~Staging() { release(); }
+    void release()
+    {
+        if (!staged) return;
+        void* ptrs[7] = {dev.lnW, dev.alive, dev.m_seq, dev.digest, dev.conf, dev.ree2, dev.rg2};
+        for (void* q : ptrs) if (q) cudaFreeAsync(q, stream);
+        staged = false;
+    }
+};
+
+int stage_outputs(const rosen_outputs* o, const Sizes& z, cudaStream_t stream, Staging* st)
+{
+    st->stream = stream;
+    if (!o) return ROSEN_OK;
+    if (o->memory == ROSEN_MEM_DEVICE) {
+        st->dev = DevOutputs{o->lnW, o->alive, o->m_seq, o->digest, o->conf, o->ree2, o->rg2};
+        return ROSEN_OK;
+    }
+    if (o->memory != ROSEN_MEM_HOST) { std::snprintf(g_err, sizeof(g_err), "outputs->memory must be ROSEN_MEM_DEVICE or ROSEN_MEM_HOST"); return ROSEN_EINVAL; }
+    st->staged = true;
+    auto alloc = [&](const void* host, size_t bytes, void** d) -> int {
+        *d = nullptr;
+        if (!host) return ROSEN_OK;
+        cudaError_t e = cudaMallocAsync(d, bytes, stream);
+        if (e != cudaSuccess) { fail_cuda(e, "cudaMallocAsync(staging)"); return ROSEN_ENOMEM; }
+        return ROSEN_OK;
+    };
+    int rc;
+    if ((rc = alloc(o->lnW, z.lnW, (void**)&st->dev.lnW))) return rc;
+    if ((rc = alloc(o->alive, z.alive, (void**)&st->dev.alive))) return rc;
+    if ((rc = alloc(o->m_seq, z.m_seq, (void**)&st->dev.m_seq))) return rc;
+    if ((rc = alloc(o->digest, z.digest, (void**)&st->dev.digest))) return rc;
+    if ((rc = alloc(o->conf, z.conf, (void**)&st->dev.conf))) return rc;
+    if ((rc = alloc(o->ree2, z.ree2, (void**)&st->dev.ree2))) return rc;
+    if ((rc = alloc(o->rg2, z.rg2, (void**)&st->dev.rg2))) return rc;
+    return ROSEN_OK;
+}
+
+int copy_back(const rosen_outputs* o, const Sizes& z, const Staging& st, cudaStream_t stream)
+{
+    if (!o || !st.staged) return ROSEN_OK;
+    if (o->lnW) CK(cudaMemcpyAsync(o->lnW, st.dev.lnW, z.lnW, cudaMemcpyDeviceToHost, stream));
+    if (o->alive) CK(cudaMemcpyAsync(o->alive, st.dev.alive, z.alive, cudaMemcpyDeviceToHost, stream));
+    if (o->m_seq) CK(cudaMemcpyAsync(o->m_seq, st.dev.m_seq, z.m_seq, cudaMemcpyDeviceToHost, stream));
+    if (o->digest) CK(cudaMemcpyAsync(o->digest, st.dev.digest, z.digest, cudaMemcpyDeviceToHost, stream));
+    if (o->conf) CK(cudaMemcpyAsync(o->conf, st.dev.conf, z.conf, cudaMemcpyDeviceToHost, stream));
+    if (o->ree2) CK(cudaMemcpyAsync(o->ree2, st.dev.ree2, z.ree2, cudaMemcpyDeviceToHost, stream));
+    if (o->rg2) CK(cudaMemcpyAsync(o->rg2, st.dev.rg2, z.rg2, cudaMemcpyDeviceToHost, stream));
+    return ROSEN_OK;
+}
+
+void derive(rosen_summary* s)
+{
+    s->mean_ree2 = s->sum_w_ree2 / s->sum_w;
+    s->mean_rg2 = s->sum_w_rg2 / s->sum_w;
+    s->attrition = (double)s->n_dead / (double)s->n_chains;
+    s->ln_mean_W = s->ln_shift + std::log(s->sum_w / (double)s->n_chains);
+}
+
+// After the generation kernel: second reduction pass, summary copy, host staging copies, sync.
+int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const rosen_outputs* outputs, const Sizes& z,
+           Staging& st, rosen_summary* summary, cudaStream_t stream)
+{
+    if (summary) {
+        if (rosen::launch_finalize(sc->dev, grid, sc->dev + rosen::kMaxPartials, stream) < 0) return fail_cuda(cudaGetLastError(), "finalize_kernel");
+        ++g_launches;
+        CK(cudaMemcpyAsync(sc->host, sc->dev + rosen::kMaxPartials, sizeof(Partial), cudaMemcpyDeviceToHost, stream));
+    }
+    int rc = copy_back(outputs, z, st, stream);
+    if (rc) return rc;
+    st.release();
+    if (summary || (outputs && outputs->memory == ROSEN_MEM_HOST)) CK(cudaStreamSynchronize(stream));
+    if (summary) {
+        const Partial& t = *sc->host;
+        summary->n_chains = n_chains; summary->n_dead = t.n_dead; summary->n_steps_attempted = t.n_steps;
+        summary->ln_shift = ln_shift;
+        summary->sum_w = t.sum_w; summary->sum_w_ree2 = t.sum_w_ree2; summary->sum_w_rg2 = t.sum_w_rg2; summary->sum_w2 = t.sum_w2;
+        summary->digest_xor = t.digest_xor; summary->digest_sum = t.digest_sum;
+        derive(summary);
+    }
+    return ROSEN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                           const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_chains == 0) { std::snprintf(g_err, sizeof(g_err), "need N >= 2 and n_chains >= 1"); return ROSEN_EINVAL; }
+    if (N > ROSEN_LATTICE_MAX_N) { std::snprintf(g_err, sizeof(g_err), "lattice N > %d", ROSEN_LATTICE_MAX_N); return ROSEN_ERANGE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* sc = nullptr;
+    int rc = get_scratch(&sc);
+    if (rc) return rc;
+    const Sizes z = output_sizes(N, n_chains, sizeof(int32_t));
+    Staging st;
+    if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
+
+    rosen::LatticeParams p{};
+    p.N = N; p.n_chains = n_chains; p.chain_offset = chain_offset;
+    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
+    p.ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
+    p.out = st.dev; p.partials = sc->dev;
+    int grid = 0;
+    rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
+    if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");
+    g_launches += rc;
+    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, stream);
+}
+
+int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                             uint64_t seed, uint64_t chain_offset,
+                             const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_chains == 0 || k_trials < 1 || k_trials > 255 || !(bond_len > 0.0f) || !(sigma >= 0.0f) ||
+        !std::isfinite(bond_len) || !std::isfinite(sigma)) {
+        std::snprintf(g_err, sizeof(g_err), "need N >= 2, n_chains >= 1, 1 <= k_trials <= 255, bond_len > 0, sigma >= 0 (finite)");
+        return ROSEN_EINVAL;
+    }
+    if (N > ROSEN_REALSPACE_MAX_N) { std::snprintf(g_err, sizeof(g_err), "real-space N > %d", ROSEN_REALSPACE_MAX_N); return ROSEN_ERANGE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* sc = nullptr;
+    int rc = get_scratch(&sc);
+    if (rc) return rc;
+    const Sizes z = output_sizes(N, n_chains, sizeof(float));
+    Staging st;
+    if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
+
+    rosen::RealParams p{};
+    p.N = N; p.k = k_trials; p.n_chains = n_chains; p.chain_offset = chain_offset;
+    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
+    p.b = bond_len; p.sigma2 = sigma * sigma;   // fp32 product, rounded once
+    {   // conservative candidate radius, rounded up: ((b + sigma)(1 + 2^-9))^2
+        const double r = ((double)bond_len + (double)sigma) * (1.0 + 1.0 / 512.0);
+        float r2 = (float)(r * r);
+        if ((double)r2 < r * r) r2 = std::nextafterf(r2, INFINITY);
+        p.prefilter2 = r2;
+    }
+    p.ln_shift = (double)(N - 1) * std::log((double)k_trials);
+    p.out = st.dev; p.partials = sc->dev;
+    int grid = 0;
+    rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
+    if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space kernel launch");
+    g_launches += rc;
+    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, stream);
+}
+
+int rosen_lattice_dump(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                       int32_t* conf, double* lnW, int32_t memory, rosen_summary* summary, void* cuda_stream)
+{
+    rosen_outputs o{};
+    o.conf = conf; o.lnW = lnW; o.memory = memory;
+    return rosen_lattice_generate(N, n_chains, seed, chain_offset, &o, summary, cuda_stream);
+}
+
+int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                         uint64_t seed, uint64_t chain_offset,
+                         float* conf, double* lnW, int32_t memory, rosen_summary* summary, void* cuda_stream)
+{
+    rosen_outputs o{};
+    o.conf = conf; o.lnW = lnW; o.memory = memory;
+    return rosen_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, &o, summary, cuda_stream);
+}
+
+int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged)
+{
+    if (!parts || !merged || count < 1) return ROSEN_EINVAL;
+    rosen_summary m = parts[0];
+    for (int32_t i = 1; i < count; ++i) {
+        const rosen_summary& q = parts[i];
+        if (q.ln_shift != m.ln_shift) return ROSEN_EINVAL;
+        m.n_chains += q.n_chains; m.n_dead += q.n_dead; m.n_steps_attempted += q.n_steps_attempted;
+        m.sum_w += q.sum_w; m.sum_w_ree2 += q.sum_w_ree2; m.sum_w_rg2 += q.sum_w_rg2; m.sum_w2 += q.sum_w2;
+        m.digest_xor ^= q.digest_xor; m.digest_sum += q.digest_sum;
+    }
+    derive(&m);
+    *merged = m;
+    return ROSEN_OK;
+}
+
+size_t rosen_workspace_bytes(void) { return sizeof(Partial) * (rosen::kMaxPartials + 1); }
+int32_t rosen_last_launch_count(void) { return g_launches; }
+const char* rosen_last_kernel_name(void) { return g_kernel; }
+
+const char* rosen_strerror(int code)
+{
+    switch (code) {
+        case ROSEN_OK: return "success";
+        case ROSEN_EINVAL: return "invalid argument";
+        case ROSEN_ERANGE: return "chain length beyond the supported range";
+        case ROSEN_ECUDA: return "CUDA runtime error";
+        case ROSEN_ENOMEM: return "device allocation failed";
+        default: return "unknown error code";
+    }
+}
+const char* rosen_last_error(void) { return g_err; }
+const char* rosen_version(void) { return "rosen-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,298 @@
+// realspace.cu -- off-lattice Rosenbluth chain generation for sm_100a (steps R0-R5 of DESIGN.md 2;
+// PAPER.md:185-187 sec. 3.3.3, :202-262 Algorithm 2). A group of G lanes grows one chain: lane =
+// pair of trials (one Philox block), so the trial loop of Alg. 2 line 9 runs across lanes and the
+// free-trial count is a __ballot_sync/__popc. The chain lives in shared memory (SoA fp32).
+//
+// Exact pruning of Alg. 2 lines 13-19: a monomer farther than (b + sigma)(1 + 2^-9) from the growth
+// point r_{s-1} cannot be within sigma of any trial (every trial is b(1 +- 1e-6) away from r_{s-1}),
+// so each step first collects the few candidates inside that radius (cooperatively, lanes =
+// monomers) and tests the trials against those only. Decisions are identical to the full scan;
+// the argument with its fp32 error budget is DESIGN.md 5.2.
+//
+// All fp32 arithmetic that decides anything is written with explicit __f*_rn intrinsics in the order
+// DESIGN.md 3.3 fixes, so nvcc cannot contract or reorder it.
+#include <math_constants.h>
+#include "common.cuh"
+#include "philox.cuh"
+#include "reduce.cuh"
+
+namespace rosen {
+
+namespace {
+
+// "rngonsphere" (Alg. 2 line 10) on two Philox words -- DESIGN.md 3.3.
+__device__ __forceinline__ void direction(uint32_t wz, uint32_t wphi, float& ux, float& uy, float& uz)
+{
+    const float z = __fmaf_rn(__uint2float_rn(2u * (wz >> 9) + 1u), 0x1p-23f, -1.0f);
+    const uint32_t a = wphi >> 8;
+    const uint32_t oct = a >> 21;
+    const uint32_t f = a & 0x1FFFFFu;
+    const uint32_t g = (oct & 1u) ? (0x1FFFFFu - f) : f;
+    const float x = __fmul_rn(__uint2float_rn(2u * g + 1u), 0x1.921fb6p-23f);
+    const float x2 = __fmul_rn(x, x);
+    float p = __fmaf_rn(x2, 0x1.71de3ap-19f, -0x1.a01a02p-13f);
+    p = __fmaf_rn(x2, p, 0x1.111112p-7f);
+    p = __fmaf_rn(x2, p, -0x1.555556p-3f);
+    p = __fmul_rn(p, x2);
+    const float sn = __fmaf_rn(x, p, x);
+    float q = __fmaf_rn(x2, -0x1.27e4fcp-22f, 0x1.a01a02p-16f);
+    q = __fmaf_rn(x2, q, -0x1.6c16c2p-10f);
+    q = __fmaf_rn(x2, q, 0x1.555556p-5f);
+    q = __fmaf_rn(x2, q, -0.5f);
+    const float cs = __fmaf_rn(x2, q, 1.0f);
+    const bool swap = (((oct + 1u) >> 1) & 1u) != 0u;
+    float cx = swap ? sn : cs;
+    float sy = swap ? cs : sn;
+    if (oct >= 2u && oct <= 5u) cx = -cx;
+    if (oct >= 4u) sy = -sy;
+    const float rho = __fsqrt_rn(__fmaf_rn(-z, z, 1.0f));
+    ux = __fmul_rn(rho, cx); uy = __fmul_rn(rho, sy); uz = z;
+}
+
+__device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t choice)
+{
+    return (h ^ (uint64_t)(m | (choice << 8))) * 0x100000001B3ull;
+}
+
+// shared memory carve-up (bytes) -----------------------------------------------------------------
+//   double   ln_tab[256]            ln m, ln_tab[0] = -inf
+//   Partial  scratch[32]
+//   per group: float x[Np], y[Np], z[Np]; uint16 cand[Np]; uint8 mseq[Np]   (Np = N rounded up to 4)
+__host__ __device__ inline int n_pad(int N) { return (N + 3) & ~3; }
+__host__ __device__ inline size_t group_bytes(int N) { return (size_t)n_pad(N) * (12 + 2 + 1) + 4; }
+
+template <int G, int P, bool DIGEST, bool TRAJ>
+__global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* ln_tab = reinterpret_cast<double*>(smem_raw);
+    Partial* scratch = reinterpret_cast<Partial*>(smem_raw + 256 * sizeof(double));
+    unsigned char* gbase_ptr = smem_raw + 256 * sizeof(double) + 32 * sizeof(Partial);
+
+    const int N = p.N, k = p.k, Np = n_pad(N);
+    const int lane = threadIdx.x & 31;
+    const int gl = lane & (G - 1);                         // lane within the group
+    const int gshift = lane & ~(G - 1);                    // first lane of the group in the warp
+    const uint32_t gmask = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    const uint32_t below = (1u << gl) - 1u;
+    const int group_in_block = threadIdx.x / G;
+    const size_t gsz = (group_bytes(N) + 15) & ~(size_t)15;
+    float* X = reinterpret_cast<float*>(gbase_ptr + gsz * group_in_block);
+    float* Y = X + Np;
+    float* Z = Y + Np;
+    uint16_t* cand = reinterpret_cast<uint16_t*>(Z + Np);
+    uint8_t* mbuf = reinterpret_cast<uint8_t*>(cand + Np);
+
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
+    __syncthreads();
+
+    Partial acc = partial_zero();
+    const uint64_t n_groups = ((uint64_t)gridDim.x * blockDim.x) / G;
+    const uint64_t first = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
+    // all groups of a warp run the same number of iterations (warp-level primitives below)
+    const uint64_t iters = (p.n_chains + n_groups - 1) / n_groups;
+
+    for (uint64_t it = 0; it < iters; ++it) {
+        const uint64_t idx = first + it * n_groups;
+        const bool active = idx < p.n_chains;               // inactive groups compute and discard
+        const uint64_t chain = p.chain_offset + idx;
+        const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
+
+        // R0
+        float hx = 0.f, hy = 0.f, hz = 0.f;
+        if (gl == 0) { X[0] = 0.f; Y[0] = 0.f; Z[0] = 0.f; }
+        double lnW = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0, S2 = 0.0;
+        bool alive = true;
+        uint32_t steps = 0;
+        uint64_t dg = 0xCBF29CE484222325ull;
+        uint32_t selw[4] = {0, 0, 0, 0};
+        __syncwarp();
+
+        for (int s = 1; s < N; ++s) {
+            if ((s & 3) == 0 || s == 1) philox4x32_10(c_lo, c_hi, (uint32_t)(s >> 2), 0u, p.key0, p.key1, selw);
+
+            // ---- candidates: monomers j <= s-2 within the conservative radius of r_{s-1}
+            int ncand = 0;
+            for (int j0 = 0; j0 < s - 1; j0 += G) {
+                const int j = j0 + gl;
+                bool in = false;
+                if (j < s - 1) {
+                    const float dx = X[j] - hx, dy = Y[j] - hy, dz = Z[j] - hz;
+                    in = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < p.prefilter2;
+                }
+                const uint32_t bits = (__ballot_sync(0xffffffffu, in) >> gshift) & gmask;
+                if (in) cand[ncand + __popc(bits & below)] = (uint16_t)j;
+                ncand += __popc(bits);
+            }
+            __syncwarp();
+
+            // ---- R1 + R2: this lane's trials (P Philox blocks = 2P trials)
+            float tx[P][2], ty[P][2], tz[P][2];
+            bool fr[P][2];
+#pragma unroll
+            for (int pp = 0; pp < P; ++pp) {
+                const uint32_t bi = (uint32_t)(gl + G * pp);
+                uint32_t w[4];
+                philox4x32_10(c_lo, c_hi, (uint32_t)s, 1u + bi, p.key0, p.key1, w);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    float ux, uy, uz;
+                    direction(w[2 * e], w[2 * e + 1], ux, uy, uz);
+                    tx[pp][e] = __fmaf_rn(p.b, ux, hx);
+                    ty[pp][e] = __fmaf_rn(p.b, uy, hy);
+                    tz[pp][e] = __fmaf_rn(p.b, uz, hz);
+                    fr[pp][e] = (int)(2u * bi + e) < k;
+                }
+            }
+            for (int c = 0; c < ncand; ++c) {
+                const int j = cand[c];
+                const float xj = X[j], yj = Y[j], zj = Z[j];
+#pragma unroll
+                for (int pp = 0; pp < P; ++pp)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const float dx = __fsub_rn(xj, tx[pp][e]), dy = __fsub_rn(yj, ty[pp][e]), dz = __fsub_rn(zj, tz[pp][e]);
+                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                        if (d2 < p.sigma2) fr[pp][e] = false;
+                    }
+            }
+
+            // ---- m_s and the rank of each free trial in trial order t = 2*(gl + G*pp) + e
+            uint32_t B[P][2];
+            uint32_t m = 0;
+#pragma unroll
+            for (int pp = 0; pp < P; ++pp)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    B[pp][e] = (__ballot_sync(0xffffffffu, fr[pp][e]) >> gshift) & gmask;
+                    m += __popc(B[pp][e]);
+                }
+
+            // ---- R3
+            steps += alive ? 1u : 0u;
+            lnW += ln_tab[m];
+            if (TRAJ) { if (gl == 0) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
+
+            // ---- R4: the sel-th free trial
+            const uint32_t sel = __umulhi(selw[s & 3], m);
+            uint32_t base = 0;
+            bool hit = false;
+            float px = hx, py = hy, pz = hz;
+            uint32_t tsel = 0;
+#pragma unroll
+            for (int pp = 0; pp < P; ++pp) {
+                const uint32_t r0 = base + __popc(B[pp][0] & below) + __popc(B[pp][1] & below);
+                const uint32_t r1 = r0 + (fr[pp][0] ? 1u : 0u);
+                if (fr[pp][0] && r0 == sel) { hit = true; px = tx[pp][0]; py = ty[pp][0]; pz = tz[pp][0]; tsel = 2u * (gl + G * pp); }
+                if (fr[pp][1] && r1 == sel) { hit = true; px = tx[pp][1]; py = ty[pp][1]; pz = tz[pp][1]; tsel = 2u * (gl + G * pp) + 1u; }
+                base += __popc(B[pp][0]) + __popc(B[pp][1]);
+            }
+            const uint32_t hb = (__ballot_sync(0xffffffffu, hit) >> gshift) & gmask;
+            const int src = gshift + (hb ? __ffs(hb) - 1 : 0);
+            px = __shfl_sync(0xffffffffu, px, src); py = __shfl_sync(0xffffffffu, py, src);
+            pz = __shfl_sync(0xffffffffu, pz, src); tsel = __shfl_sync(0xffffffffu, tsel, src);
+            if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? tsel : 0xFFu); }
+            alive = alive && (m != 0u);
+            if (m != 0u) { hx = px; hy = py; hz = pz; }
+            if (gl == 0) { X[s] = hx; Y[s] = hy; Z[s] = hz; }
+
+            // ---- R5 running sums (fp64)
+            Sx += (double)hx; Sy += (double)hy; Sz += (double)hz;
+            S2 += (double)hx * (double)hx + (double)hy * (double)hy + (double)hz * (double)hz;
+            __syncwarp();
+        }
+
+        double ree2 = 0.0, rg2 = 0.0;
+        if (alive) {
+            ree2 = (double)hx * (double)hx + (double)hy * (double)hy + (double)hz * (double)hz;
+            const double inv = 1.0 / (double)N;
+            const double cx = Sx * inv, cy = Sy * inv, cz = Sz * inv;
+            rg2 = S2 * inv - (cx * cx + cy * cy + cz * cz);
+        }
+        const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
+        if (active && gl == 0) {
+            acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
+            acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
+            if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
+            if (p.out.lnW) p.out.lnW[idx] = lnW;
+            if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
+            if (p.out.ree2) p.out.ree2[idx] = ree2;
+            if (p.out.rg2) p.out.rg2[idx] = rg2;
+            if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
+        }
+        if (TRAJ && active) {
+            // D1: the group streams its chain out of shared memory, interleaving SoA -> [N][3]
+            const int placed = alive ? N : (int)steps;
+            if (p.out.conf) {
+                float* c = reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3;
+                for (int e = gl; e < 3 * N; e += G) {
+                    const int i = e / 3, a = e - 3 * i;
+                    const float v = a == 0 ? X[i] : (a == 1 ? Y[i] : Z[i]);
+                    c[e] = i < placed ? v : 0.0f;
+                }
+            }
+            if (p.out.m_seq) {
+                uint8_t* mr = p.out.m_seq + idx * (uint64_t)(N - 1);
+                for (int e = gl; e < N - 1; e += G) mr[e] = mbuf[e];
+            }
+        }
+        __syncwarp();
+    }
+
+    block_reduce_store(acc, scratch, p.partials + blockIdx.x);
+}
+
+template <int G, int P, bool DIGEST, bool TRAJ>
+int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
+{
+    int dev = 0, n_sm = 0, smem_max = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
+    const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
+    int threads = 256;
+    while (threads > 32 && fixed + gsz * (threads / G) > (size_t)(100 * 1024)) threads >>= 1;
+    const size_t smem = fixed + gsz * (threads / G);
+    if (smem > (size_t)smem_max) return -2;
+    auto kern = realspace_kernel<G, P, DIGEST, TRAJ>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
+    const uint64_t groups_per_block = threads / G;
+    uint64_t want = (p.n_chains + groups_per_block - 1) / groups_per_block;
+    uint64_t cap = (uint64_t)n_sm * per_sm;
+    if (cap > (uint64_t)kMaxPartials) cap = kMaxPartials;
+    const int grid = (int)(want < cap ? want : cap);
+    kern<<<grid, threads, smem, stream>>>(p);
+    if (cudaGetLastError() != cudaSuccess) return -3;
+    *grid_out = grid;
+    return 1;
+}
+
+template <int G, int P>
+int launch_gp(const RealParams& p, cudaStream_t stream, int* grid_out)
+{
+    const bool digest = p.out.digest != nullptr;
+    const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
+    if (traj) return digest ? launch_one<G, P, true, true>(p, stream, grid_out) : launch_one<G, P, false, true>(p, stream, grid_out);
+    return digest ? launch_one<G, P, true, false>(p, stream, grid_out) : launch_one<G, P, false, false>(p, stream, grid_out);
+}
+
+}  // namespace
+
+int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out)
+{
+    const int blocks = (p.k + 1) / 2;   // Philox blocks (trial pairs) per step
+    if (blocks <= 1)  { *kernel_name = "realspace_kernel<G=1,P=1>";  return launch_gp<1, 1>(p, stream, grid_out); }
+    if (blocks <= 2)  { *kernel_name = "realspace_kernel<G=2,P=1>";  return launch_gp<2, 1>(p, stream, grid_out); }
+    if (blocks <= 4)  { *kernel_name = "realspace_kernel<G=4,P=1>";  return launch_gp<4, 1>(p, stream, grid_out); }
+    if (blocks <= 8)  { *kernel_name = "realspace_kernel<G=8,P=1>";  return launch_gp<8, 1>(p, stream, grid_out); }
+    if (blocks <= 16) { *kernel_name = "realspace_kernel<G=16,P=1>"; return launch_gp<16, 1>(p, stream, grid_out); }
+    if (blocks <= 32) { *kernel_name = "realspace_kernel<G=32,P=1>"; return launch_gp<32, 1>(p, stream, grid_out); }
+    if (blocks <= 64) { *kernel_name = "realspace_kernel<G=32,P=2>"; return launch_gp<32, 2>(p, stream, grid_out); }
+    *kernel_name = "realspace_kernel<G=32,P=4>";
+    return launch_gp<32, 4>(p, stream, grid_out);
+}
+
+}  // namespace rosen

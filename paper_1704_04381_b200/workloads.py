@@ -1,0 +1,46 @@
+"""The synthetic workloads of BASELINE.json `configs` -- parameters only, no arithmetic of the method.
+
+The path has no input arrays: a workload is (N, n_chains, seed, ...) and every random number is
+drawn inside the path from the counter-based generator keyed by (seed, chain id, step). This
+module is the single "input generator" shared by tests, bench.py, the CUDA binding callers and the
+oracle callers; it imports neither of them.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional, Tuple
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    kind: str                 # "lattice" | "realspace"
+    N: int
+    n_chains: int
+    seed: int
+    k_trials: Optional[int] = None
+    bond_len: Optional[float] = None
+    sigma: Optional[float] = None
+    dump: bool = False        # full per-chain conformation output (config 5)
+
+    def monomer_steps_nominal(self) -> int:
+        return self.n_chains * (self.N - 1)
+
+
+# BASELINE.json configs[0..4]; config 3 has no seed in BASELINE.json: seed = 3.
+CONFIG_1 = Workload("lattice_N16_2p16", "lattice", 16, 1 << 16, 1)
+CONFIG_2 = Workload("lattice_N64_2p24", "lattice", 64, 1 << 24, 7)
+CONFIG_3 = Workload("realspace_N64_k16_2p22", "realspace", 64, 1 << 22, 3, 16, 1.0, 1.0)
+CONFIG_4_N: Tuple[int, ...] = (8, 16, 32, 64, 128, 256)
+CONFIG_4 = tuple(Workload(f"lattice_sweep_N{N}_2p24", "lattice", N, 1 << 24, 11) for N in CONFIG_4_N)
+CONFIG_5 = Workload("realspace_N256_k64_2p20_dump", "realspace", 256, 1 << 20, 13, 64, 1.0, 0.8, dump=True)
+
+CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5)}
+
+
+def shard(n_chains: int, rank: int, world: int) -> Tuple[int, int]:
+    """Contiguous chain-id range [offset, offset+count) of `rank` among `world` ranks (balanced)."""
+    base, rem = divmod(n_chains, world)
+    count = base + (1 if rank < rem else 0)
+    offset = rank * base + min(rank, rem)
+    return offset, count

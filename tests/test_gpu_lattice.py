@@ -1,0 +1,163 @@
+"""GPU parity: CUDA lattice path (through the C ABI) vs the CPU oracle, element by element.
+
+Bar (BASELINE north_star): trajectory, m_i sequence, dead/alive flag bit-exact per chain; ensemble
+fp64 sums within 1e-12 relative.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1704_04381_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-12
+ALL = ("lnW", "alive", "m_seq", "digest", "conf", "ree2", "rg2")
+
+
+@pytest.fixture(scope="module")
+def R():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1704_04381_b200 as R
+    R.load_library()
+    return R
+
+
+def compare_per_chain(t, o, N):
+    conf = t["conf"].cpu().numpy()
+    assert np.array_equal(conf, o.conf), "trajectory mismatch"
+    assert np.array_equal(t["m_seq"].cpu().numpy(), o.m_seq), "m sequence mismatch"
+    assert np.array_equal(t["alive"].cpu().numpy(), o.alive), "alive flag mismatch"
+    assert np.array_equal(t["digest"].cpu().numpy().view(np.uint64), o.digest), "digest mismatch"
+    lnW = t["lnW"].cpu().numpy()
+    dead = o.alive == 0
+    assert np.all(np.isneginf(lnW[dead]))
+    assert np.allclose(lnW[~dead], o.lnW[~dead], rtol=REL, atol=0)
+    assert np.array_equal(t["ree2"].cpu().numpy(), o.ree2)          # integers: exact
+    assert np.allclose(t["rg2"].cpu().numpy(), o.rg2, rtol=REL, atol=0)
+
+
+def compare_summary(s, so):
+    for key in ("n_chains", "n_dead", "n_steps_attempted", "digest_xor", "digest_sum"):
+        assert s[key] == so[key], key
+    for key in ("ln_shift", "sum_w", "sum_w_ree2", "sum_w_rg2", "sum_w2", "mean_ree2", "mean_rg2", "attrition", "ln_mean_W"):
+        assert math.isclose(s[key], so[key], rel_tol=REL, abs_tol=0.0), (key, s[key], so[key])
+
+
+def test_config1_full_parity(R):
+    w = workloads.CONFIG_1
+    s, t = R.rosen_lattice_generate(w.N, w.n_chains, w.seed, outputs=ALL)
+    o = oracle.lattice_generate(w.N, w.n_chains, w.seed)
+    compare_per_chain(t, o, w.N)
+    compare_summary(s, o.summary)
+    assert "lattice" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 2
+
+
+@pytest.mark.parametrize("N,n_chains,seed,offset", [
+    (2, 1, 0, 0), (2, 1000, 5, 7), (3, 33, 1, 0), (4, 257, 2, 0), (5, 4099, 3, 1 << 40),
+    (9, 5000, 4, (1 << 32) - 100), (17, 3001, 8, 0), (33, 2049, 9, 0), (64, 9001, 7, 12345),
+    (65, 777, 7, 0), (127, 1500, 11, 0), (128, 1500, 11, 0), (129, 700, 11, 0), (200, 900, 12, 0),
+    (256, 1200, 11, 3), (300, 300, 13, 0), (512, 200, 14, 0),
+])
+def test_shapes_ragged_and_edges(R, N, n_chains, seed, offset):
+    s, t = R.rosen_lattice_generate(N, n_chains, seed, chain_offset=offset, outputs=ALL)
+    o = oracle.lattice_generate(N, n_chains, seed, chain_offset=offset)
+    compare_per_chain(t, o, N)
+    compare_summary(s, o.summary)
+
+
+def test_summary_only_variant_is_bit_identical_and_deterministic(R):
+    N, n, seed = 64, 100003, 7
+    s0, _ = R.rosen_lattice_generate(N, n, seed)
+    s1, _ = R.rosen_lattice_generate(N, n, seed)
+    assert s0 == s1
+    s2, t = R.rosen_lattice_generate(N, n, seed, outputs=("lnW", "ree2", "rg2", "alive"))
+    for k in s0:
+        if not k.startswith("digest"):
+            assert s0[k] == s2[k], k
+    s3, _ = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
+    for k in s0:
+        if not k.startswith("digest"):
+            assert s0[k] == s3[k], k
+    o = oracle.lattice_generate(N, n, seed, outputs=("digest",))
+    compare_summary(s3, o.summary)
+
+
+def test_host_outputs_and_dump_entry_points(R):
+    N, n, seed = 24, 5000, 21
+    s_d, t_d = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
+    s_h, t_h = R.rosen_lattice_generate(N, n, seed, outputs=ALL, host_outputs=True)
+    assert s_d == s_h
+    for k in ALL:
+        assert not t_h[k].is_cuda
+        assert np.array_equal(t_d[k].cpu().numpy(), t_h[k].numpy()), k
+    s, conf, lnW = R.rosen_lattice_dump(N, n, seed)
+    assert np.array_equal(conf.cpu().numpy(), t_d["conf"].cpu().numpy())
+    assert np.array_equal(lnW.cpu().numpy(), t_d["lnW"].cpu().numpy())
+
+
+def test_chain_offset_subrange_and_merge(R):
+    N, n, seed = 32, 40000, 5
+    s_all, t_all = R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW"))
+    parts = []
+    for rank in range(3):
+        off, cnt = workloads.shard(n, rank, 3)
+        s, t = R.rosen_lattice_generate(N, cnt, seed, chain_offset=off, outputs=("digest", "lnW"))
+        assert np.array_equal(t["digest"].cpu().numpy(), t_all["digest"][off:off + cnt].cpu().numpy())
+        parts.append(s)
+    m = R.rosen_summary_merge(parts)
+    for key in ("n_chains", "n_dead", "n_steps_attempted", "digest_xor", "digest_sum"):
+        assert m[key] == s_all[key]
+    for key in ("sum_w", "sum_w_ree2", "sum_w_rg2", "sum_w2", "mean_ree2", "mean_rg2", "ln_mean_W"):
+        assert math.isclose(m[key], s_all[key], rel_tol=1e-13)
+
+
+def test_error_codes(R):
+    for args, code in [((1, 10, 0), R.ROSEN_EINVAL), ((8, 0, 0), R.ROSEN_EINVAL), ((513, 10, 0), R.ROSEN_ERANGE)]:
+        with pytest.raises(R.RosenError) as e:
+            R.rosen_lattice_generate(*args)
+        assert e.value.code == code
+
+
+def test_config2_full_size_sampled(R):
+    """BASELINE config 2 at full size in the launch configuration bench.py times (summary only),
+    plus the same launch with per-chain scalars for sampled one-by-one oracle checks and
+    size-independent properties."""
+    import torch
+    w = workloads.CONFIG_2
+    s_bench, _ = R.rosen_lattice_generate(w.N, w.n_chains, w.seed)
+    name_bench = R.rosen_last_kernel_name()
+    s, t = R.rosen_lattice_generate(w.N, w.n_chains, w.seed, outputs=("lnW", "alive", "ree2", "rg2", "digest"))
+    for k in s_bench:
+        if not k.startswith("digest"):
+            assert s_bench[k] == s[k], k                      # same reduction tree, bit-identical
+    assert name_bench.startswith("lattice")
+    # contiguous prefix + scattered samples, one by one against the oracle
+    pre = 1 << 15
+    o = oracle.lattice_generate(w.N, pre, w.seed, outputs=("lnW", "alive", "ree2", "rg2", "digest"))
+    assert np.array_equal(t["digest"][:pre].cpu().numpy().view(np.uint64), o.digest)
+    assert np.array_equal(t["alive"][:pre].cpu().numpy(), o.alive)
+    assert np.array_equal(t["ree2"][:pre].cpu().numpy(), o.ree2)
+    rng = np.random.default_rng(2024)
+    ids = np.unique(np.concatenate([rng.integers(0, w.n_chains, 2000), [w.n_chains - 1, w.n_chains - 2]]))
+    dg = t["digest"].cpu().numpy().view(np.uint64); lw = t["lnW"].cpu().numpy(); rg = t["rg2"].cpu().numpy()
+    for i in ids:
+        oi = oracle.lattice_generate(w.N, 1, w.seed, chain_offset=int(i), outputs=("lnW", "rg2", "digest"))
+        assert oi.digest[0] == dg[i]
+        assert (np.isneginf(lw[i]) and np.isneginf(oi.lnW[0])) or math.isclose(lw[i], oi.lnW[0], rel_tol=REL)
+        assert math.isclose(rg[i], oi.rg2[0], rel_tol=REL)
+    # properties at full size: the summary is the reduction of the per-chain outputs
+    alive = t["alive"].bool()
+    wgt = torch.where(alive, torch.exp(t["lnW"] - s["ln_shift"]), torch.zeros_like(t["lnW"]))
+    assert int((~alive).sum()) == s["n_dead"]
+    assert math.isclose(float(wgt.sum()), s["sum_w"], rel_tol=1e-11)
+    assert math.isclose(float((wgt * t["ree2"]).sum()), s["sum_w_ree2"], rel_tol=1e-11)
+    assert math.isclose(float((wgt * t["rg2"]).sum()), s["sum_w_rg2"], rel_tol=1e-11)
+    d64 = t["digest"]
+    assert int(d64.sum()) & (2 ** 64 - 1) == s["digest_sum"]     # int64 wrap-around sum == uint64 sum mod 2^64
+    # physics sanity (loose): attrition ~3.6e-3, nu-consistent <Ree2> ~ 152
+    assert 2e-3 < s["attrition"] < 6e-3 and 140 < s["mean_ree2"] < 165

@@ -1,0 +1,136 @@
+"""GPU parity: CUDA real-space path (through the C ABI) vs the CPU oracle.
+
+Bar (BASELINE north_star): coordinates within 1e-5 absolute in fp32 (expected: identical bits,
+the arithmetic is specified to the operation), fraction of chains whose overlap decision flips
+< 1e-4 (expected 0; measured via the per-chain decision digest), ensemble averages within 1e-6.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1704_04381_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+ALL = ("lnW", "alive", "m_seq", "digest", "conf", "ree2", "rg2")
+
+
+@pytest.fixture(scope="module")
+def R():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1704_04381_b200 as R
+    R.load_library()
+    return R
+
+
+def check(R, N, n, k, b, sigma, seed, offset=0, exact=True):
+    s, t = R.rosen_realspace_generate(N, n, k, b, sigma, seed, chain_offset=offset, outputs=ALL)
+    o = oracle.realspace_generate(N, n, k, b, sigma, seed, chain_offset=offset)
+    dg = t["digest"].cpu().numpy().view(np.uint64)
+    flips = float((dg != o.digest).mean())
+    assert flips < 1e-4, f"flip fraction {flips}"
+    same = dg == o.digest
+    conf = t["conf"].cpu().numpy()
+    assert np.abs(conf[same] - o.conf[same]).max(initial=0.0) <= 1e-5
+    if exact:   # by construction the two sides execute the same IEEE operations
+        assert flips == 0.0
+        assert np.array_equal(conf, o.conf)
+        assert np.array_equal(t["m_seq"].cpu().numpy(), o.m_seq)
+        assert np.array_equal(t["alive"].cpu().numpy(), o.alive)
+        lnW = t["lnW"].cpu().numpy()
+        dead = o.alive == 0
+        assert np.all(np.isneginf(lnW[dead])) and np.allclose(lnW[~dead], o.lnW[~dead], rtol=1e-13, atol=0)
+        assert np.allclose(t["ree2"].cpu().numpy(), o.ree2, rtol=1e-12, atol=0)
+        assert np.allclose(t["rg2"].cpu().numpy(), o.rg2, rtol=1e-9, atol=0)
+        for key in ("n_chains", "n_dead", "n_steps_attempted", "digest_xor", "digest_sum"):
+            assert s[key] == o.summary[key], key
+    for key in ("sum_w", "sum_w_ree2", "sum_w_rg2", "sum_w2", "mean_ree2", "mean_rg2", "ln_mean_W"):
+        both_nan = math.isnan(s[key]) and math.isnan(o.summary[key])      # every chain dead: 0/0 on both sides
+        assert both_nan or math.isclose(s[key], o.summary[key], rel_tol=1e-6), (key, s[key], o.summary[key])
+    return flips
+
+
+def test_config3_prefix(R):
+    w = workloads.CONFIG_3
+    check(R, w.N, 1 << 13, w.k_trials, w.bond_len, w.sigma, w.seed)
+
+
+def test_config5_prefix(R):
+    w = workloads.CONFIG_5
+    check(R, w.N, 192, w.k_trials, w.bond_len, w.sigma, w.seed)
+
+
+@pytest.mark.parametrize("N,n,k,b,sigma,seed,offset", [
+    (2, 1, 1, 1.0, 1.0, 0, 0), (2, 100, 5, 1.0, 1.0, 1, 0), (3, 3000, 16, 1.0, 1.0, 3, 0),
+    (8, 1000, 1, 1.0, 0.5, 4, 0), (8, 1000, 2, 1.0, 0.9, 4, 9), (9, 777, 3, 1.5, 1.0, 5, 0),
+    (16, 1001, 4, 1.0, 1.0, 6, 0), (16, 999, 7, 0.7, 1.0, 6, (1 << 32) - 5), (20, 600, 8, 1.0, 1.2, 7, 0),
+    (33, 500, 9, 1.0, 1.0, 8, 0), (33, 500, 16, 1.0, 0.0, 8, 0), (40, 400, 17, 1.0, 1.0, 9, 0),
+    (40, 300, 32, 2.0, 1.7, 9, 0), (31, 300, 33, 1.0, 1.0, 10, 0), (25, 300, 64, 1.0, 1.0, 10, 0),
+    (25, 200, 65, 1.0, 0.8, 11, 0), (20, 150, 128, 1.0, 1.0, 11, 0), (18, 100, 129, 1.0, 1.0, 12, 0),
+    (12, 100, 255, 1.0, 1.0, 12, 0), (130, 64, 16, 1.0, 1.0, 13, 0), (64, 2000, 16, 1.0, 1.9, 14, 0),
+])
+def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
+    check(R, N, n, k, b, sigma, seed, offset)
+
+
+def test_summary_only_variant_bit_identical(R):
+    N, n, k = 32, 20011, 16
+    s0, _ = R.rosen_realspace_generate(N, n, k, 1.0, 1.0, 3)
+    s1, _ = R.rosen_realspace_generate(N, n, k, 1.0, 1.0, 3)
+    assert s0 == s1
+    s2, _ = R.rosen_realspace_generate(N, n, k, 1.0, 1.0, 3, outputs=ALL)
+    for key in s0:
+        if not key.startswith("digest"):
+            assert s0[key] == s2[key], key
+
+
+def test_dump_entry_point_and_host_outputs(R):
+    N, n, k = 48, 3000, 16
+    s, t = R.rosen_realspace_generate(N, n, k, 1.0, 0.8, 13, outputs=("conf", "lnW"))
+    s2, conf, lnW = R.rosen_realspace_dump(N, n, k, 1.0, 0.8, 13)
+    assert np.array_equal(conf.cpu().numpy(), t["conf"].cpu().numpy())
+    assert np.array_equal(lnW.cpu().numpy(), t["lnW"].cpu().numpy())
+    s3, th = R.rosen_realspace_generate(N, n, k, 1.0, 0.8, 13, outputs=("conf", "lnW"), host_outputs=True)
+    assert np.array_equal(th["conf"].numpy(), t["conf"].cpu().numpy())
+    assert s == s3
+
+
+def test_error_codes(R):
+    bad = [((1, 10, 4, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 0, 1.0, 1.0, 0), R.ROSEN_EINVAL),
+           ((8, 10, 256, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, 0.0, 1.0, 0), R.ROSEN_EINVAL),
+           ((8, 10, 4, 1.0, -1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, float("nan"), 1.0, 0), R.ROSEN_EINVAL),
+           ((1025, 10, 4, 1.0, 1.0, 0), R.ROSEN_ERANGE)]
+    for args, code in bad:
+        with pytest.raises(R.RosenError) as e:
+            R.rosen_realspace_generate(*args)
+        assert e.value.code == code
+
+
+def test_config3_full_size_sampled(R):
+    """Config 3 at full size (2^22 chains) in the bench launch configuration; sampled chains are
+    re-generated one by one by the oracle; physics sanity on the ensemble."""
+    w = workloads.CONFIG_3
+    s_bench, _ = R.rosen_realspace_generate(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed)
+    s, t = R.rosen_realspace_generate(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed,
+                                      outputs=("lnW", "digest", "ree2", "alive"))
+    for key in s_bench:
+        if not key.startswith("digest"):
+            assert s_bench[key] == s[key], key
+    rng = np.random.default_rng(99)
+    ids = np.unique(np.concatenate([rng.integers(0, w.n_chains, 600), [0, w.n_chains - 1]]))
+    dg = t["digest"].cpu().numpy().view(np.uint64); lw = t["lnW"].cpu().numpy(); re = t["ree2"].cpu().numpy()
+    flips = 0
+    for i in ids:
+        oi = oracle.realspace_generate(w.N, 1, w.k_trials, w.bond_len, w.sigma, w.seed, chain_offset=int(i),
+                                       outputs=("lnW", "digest", "ree2"))
+        if oi.digest[0] != dg[i]:
+            flips += 1
+            continue
+        assert (np.isneginf(lw[i]) and np.isneginf(oi.lnW[0])) or math.isclose(lw[i], oi.lnW[0], rel_tol=1e-13)
+        assert math.isclose(re[i], oi.ree2[0], rel_tol=1e-12, abs_tol=1e-12)
+    assert flips == 0
+    assert 0.01 < s["attrition"] < 0.03 and 180 < s["mean_ree2"] < 230     # 1.7 %, ~201
