@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Rosenbluth chain-generation hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+A "step" is one pass of the whole hot path (L0-L5 + E1, or R0-R5 + E1 [+ D1]) over one
+batch of the workload, i.e. one rosen_*_generate call. Default workload = BASELINE.json configs[1]
+(cubic lattice, N = 64, 2^24 chains, seed 7), the configuration the metric is quoted on.
+
+  value      chains/s, device-timed (CUDA events on the launching stream), outputs resident in HBM
+             (rosen_*_generate_async: generation kernel + second reduction pass, no host sync)
+  e2e        the same metric through the synchronous C-ABI call with HOST buffers (summary struct, and for
+             the dump workload the conformations) -- device->host copies inside the timed region
+  roofline   bound "alu": algorithmic warp-instructions / live kernel time vs issue-slot peak
+  cpu_baseline  the oracle as it stands, single thread, on a bounded sample of the same workload
+
+N > 1 (torchrun): chains are independent, so every rank generates its own n_chains with
+chain_offset = rank * n_chains (weak scaling, no data-path collective); summaries are merged on
+the host after the timed region (rosen_summary_merge).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1704_04381_b200 import workloads  # noqa: E402  (parameters only)
+
+DEFAULT_WORKLOAD = workloads.CONFIG_2.name
+METRIC = "chains/sec and monomer-steps/sec at N=64 (1 B200); % SM issue-slot peak"
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic work model -- thread-instructions the METHOD needs per chain
+# ------------------------------------------------------------------------------------------------
+def lattice_site_tests(N: int) -> int:
+    """Site tests per chain after the exact bipartite + back-site reduction: sum_s max(0, floor(s/2) - 1)."""
+    return sum(max(0, s // 2 - 1) for s in range(1, N))
+
+
+def algorithmic_thread_instr(w: workloads.Workload) -> float:
+    if w.kind == "lattice":
+        # 6 equality tests per site test + one Philox block (~70 instr) per 4 steps + ~20 per step for
+        # count / weight / choose / place / observables
+        return 6.0 * lattice_site_tests(w.N) + 70.0 * ((w.N + 3) // 4) + 20.0 * (w.N - 1)
+    # real space, full pair scan of Alg. 2: k (N-1)(N-2)/2 pair tests x 7 instr + k/2 Philox blocks and k
+    # direction evaluations (~45 instr) per step + ~30 per step
+    k, N = w.k_trials, w.N
+    pairs = k * (N - 1) * (N - 2) / 2.0
+    return 7.0 * pairs + (N - 1) * (35.0 * k + 45.0 * k + 30.0)
+
+
+def load_measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------
+# clock sampling during the timed region (B200_PROFILING.md "clocks line")
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [ln for (t, ln) in self.lines if t0 <= t <= t1 + 0.1] or [ln for (_, ln) in self.lines]
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in rows:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the two legs of the product path
+# ------------------------------------------------------------------------------------------------
+def make_calls(R, torch, w: workloads.Workload, offset: int, stream):
+    """Return (enqueue(summary_device_or_None), sync_call(), d2h_bytes) for workload w."""
+    dump = {}
+    host = {}
+    if w.dump:   # config 5: conformations + lnW written to HBM (D1)
+        ctype = torch.int32 if w.kind == "lattice" else torch.float32
+        dump = {"conf": torch.empty((w.n_chains, w.N, 3), dtype=ctype, device="cuda"),
+                "lnW": torch.empty((w.n_chains,), dtype=torch.float64, device="cuda")}
+    d2h = R.SUMMARY_BYTES + sum(t.numel() * t.element_size() for t in dump.values())
+
+    if w.kind == "lattice":
+        def enqueue(summary_device):
+            R.rosen_lattice_generate_async(w.N, w.n_chains, w.seed, offset, outputs=dump,
+                                           summary_device=summary_device, stream=stream)
+
+        def sync_call():
+            s, t = R.rosen_lattice_generate(w.N, w.n_chains, w.seed, offset, outputs=tuple(dump), stream=stream,
+                                            host_outputs=True, host_buffers=host)
+            return s
+    else:
+        def enqueue(summary_device):
+            R.rosen_realspace_generate_async(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, offset,
+                                             outputs=dump, summary_device=summary_device, stream=stream)
+
+        def sync_call():
+            s, t = R.rosen_realspace_generate(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, offset,
+                                              outputs=tuple(dump), stream=stream, host_outputs=True, host_buffers=host)
+            return s
+    return enqueue, sync_call, d2h
+
+
+def oracle_call(w: workloads.Workload, n_chains: int, offset: int = 0):
+    import oracle  # test infrastructure; allowed here for cpu_baseline / --impl reference only
+    if w.kind == "lattice":
+        return oracle.lattice_generate(w.N, n_chains, w.seed, chain_offset=offset, outputs=())
+    return oracle.realspace_generate(w.N, n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, chain_offset=offset,
+                                     outputs=())
+
+
+def time_oracle(w: workloads.Workload, target_s: float):
+    """Single-thread oracle on a chain-id prefix sized for about target_s seconds."""
+    probe = 64
+    while True:
+        t0 = time.perf_counter(); oracle_call(w, probe); dt = time.perf_counter() - t0
+        if dt > 0.2 or probe >= w.n_chains:
+            break
+        probe *= 4
+    m = int(min(w.n_chains, max(probe, probe * target_s / max(dt, 1e-9))))
+    t0 = time.perf_counter(); res = oracle_call(w, m); dt = time.perf_counter() - t0
+    return m, dt, res.summary
+
+
+def run_reference(args, w, rank):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    warmup, steps = max(args.warmup, 1), args.steps
+    m0, dt0, _ = time_oracle(w, 1.0)
+    budget = 120.0 / (steps + warmup)                    # whole run within a few minutes
+    m = int(max(16, min(w.n_chains, m0 / dt0 * min(budget, 2.0))))
+    for _ in range(warmup):
+        oracle_call(w, m)
+    t0 = time.perf_counter()
+    n_steps = 0
+    for i in range(steps):
+        n_steps += oracle_call(w, m, offset=i * m).summary["n_steps_attempted"]
+    dt = time.perf_counter() - t0
+    v = steps * m / dt
+    sample = f"{m} chains per step (chain-id ranges [i*{m}, (i+1)*{m})) of {w.name}, single thread"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "chains/s", "n_gpus": args.gpus, "steps": steps,
+        "warmup": warmup, "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32+f64" if w.kind == "lattice" else "f32+f64", "data": "synthetic",
+        "config": {"workload": w.name, "kind": w.kind, "N": w.N, "chains_per_step": m, "seed": w.seed},
+        "monomer_steps_per_s": n_steps / dt,
+        "cpu_baseline": {"value": v, "unit": "chains/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "chains/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_product(args, w, rank, world, local_rank):
+    import torch
+    import paper_1704_04381_b200 as R
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    R.load_library()                                       # fails loudly if librosen.so is missing
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    warmup, steps = max(args.warmup, 3), args.steps
+    stream = torch.cuda.Stream()
+    offset = rank * w.n_chains                             # weak scaling: disjoint chain-id ranges
+    enqueue, sync_call, d2h_bytes = make_calls(R, torch, w, offset, stream)
+    summary_dev = torch.zeros(R.SUMMARY_BYTES, dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, n):
+        """n calls of fn on `stream`, each bracketed by its own event pair; L2 flushed between calls
+        outside the pairs. Returns per-call milliseconds."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        with torch.cuda.stream(stream):
+            for a, b in ev:
+                flush.fill_(1)
+                a.record(stream); fn(); b.record(stream)
+        stream.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    # ---- device-timed leg ---------------------------------------------------------------------
+    timed(lambda: enqueue(summary_dev), warmup)
+    launches_per_step = R.rosen_last_launch_count()
+    kernel_name = R.rosen_last_kernel_name()
+    sampler = ClockSampler(local_rank); sampler.start()
+    time.sleep(0.3)
+    barrier()
+    t0 = time.perf_counter()
+    ms = timed(lambda: enqueue(summary_dev), steps)
+    barrier()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    total_ms = sum(ms)
+    summary = R.summary_from_device(summary_dev)
+
+    # ---- dominant kernel alone (generation kernel, no second pass), live, same stream ------------
+    timed(lambda: enqueue(None), 2)
+    kms = timed(lambda: enqueue(None), max(3, min(steps, 10)))
+    kernel_ms = sum(kms) / len(kms)
+
+    # ---- end-to-end leg: synchronous C-ABI call, host buffers ------------------------------------
+    for _ in range(2):
+        sync_call()
+    barrier()
+    e0 = time.perf_counter()
+    for _ in range(steps):
+        s_host = sync_call()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - e0
+    barrier()
+
+    # ---- max over ranks ---------------------------------------------------------------------------
+    if dist is not None:
+        t = torch.tensor([total_ms, e2e_s, kernel_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_s, kernel_ms = (float(x) for x in t.cpu())
+        parts = [None] * world
+        dist.all_gather_object(parts, summary)
+        summary = R.rosen_summary_merge(parts)             # rank order: deterministic
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    chains_total = w.n_chains * world
+    value = chains_total * steps / (total_ms * 1e-3)
+    steps_attempted = summary["n_steps_attempted"]
+    peaks, peaks_src = load_measured_peaks()
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    sm_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    peak_winst = n_sm * 4 * sm_hz                           # 4 schedulers/SM, 1 warp-instruction/clk each
+    alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
+    achieved = alg_winst / (kernel_ms * 1e-3)
+    roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
+                "frac": achieved / peak_winst, "traffic": None, "kernel": kernel_name, "kernel_ms": kernel_ms,
+                "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
+                "algorithmic_thread_instr_per_chain": algorithmic_thread_instr(w)}
+    if clocks.get("sm_mhz"):
+        roofline["frac_at_measured_clock"] = achieved / (n_sm * 4 * clocks["sm_mhz"] * 1e6)
+
+    out = {
+        "metric": METRIC, "value": value, "unit": "chains/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": total_ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int32+f64" if w.kind == "lattice" else "f32+f64", "data": "synthetic",
+        "config": {"workload": w.name, "kind": w.kind, "N": w.N, "n_chains_per_gpu": w.n_chains, "seed": w.seed,
+                   "k_trials": w.k_trials, "bond_len": w.bond_len, "sigma": w.sigma, "dump": w.dump,
+                   "parallelism": f"chain-range sharding x{world}, no collective",
+                   "l2": "256 MiB buffer written between timed steps; the path reads no HBM input"},
+        "monomer_steps_per_s": steps_attempted * steps / (total_ms * 1e-3),
+        "monomer_steps_nominal_per_s": chains_total * (w.N - 1) * steps / (total_ms * 1e-3),
+        "summary": {k: summary[k] for k in ("mean_ree2", "mean_rg2", "attrition", "ln_mean_W", "n_dead")},
+        "clocks": clocks, "roofline": roofline,
+        "e2e": {"value": chains_total * steps / e2e_s, "unit": "chains/s", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_s / steps * 1e3,
+                "note": "no input arrays exist (parameters by value); result = host rosen_summary"
+                        + (" + host conf/lnW" if w.dump else "")},
+        "gpu_launches": launches_per_step * steps,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        m, dt, _ = time_oracle(w, args.cpu_seconds)
+        out["cpu_baseline"] = {"value": m / dt, "unit": "chains/s", "cores": 1, "kind": "oracle",
+                               "sample": f"chain ids [0, {m}) of {w.name}, {dt:.1f} s single thread"}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--impl", default="product", choices=("product", "reference"))
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    w = workloads.CONFIGS[args.workload]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, w, rank)
+    else:
+        run_product(args, w, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -110,6 +110,18 @@ ROSEN_API int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_t
                              const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
 
 /*
+ * Enqueue-only variants: same computation, but nothing is synchronised. All outputs must be device
+ * memory (outputs->memory == ROSEN_MEM_DEVICE, else ROSEN_EINVAL); `summary_device` is a DEVICE
+ * pointer (may be NULL) that the second reduction pass fills on `cuda_stream`, derived fields
+ * included. Used to time the path with inputs/outputs resident in HBM and to overlap calls.
+ */
+ROSEN_API int rosen_lattice_generate_async(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                                 const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
+ROSEN_API int rosen_realspace_generate_async(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                                   uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
+
+/*
  * Conformation dump alone (the store path of PAPER.md:80 / :189, BASELINE config 5): identical to
  * the generate calls with outputs = {conf, lnW} only, provided as named entry points.
  * conf/lnW are DEVICE pointers when memory == ROSEN_MEM_DEVICE, host pointers otherwise.

@@ -68,6 +68,11 @@ def load_library() -> C.CDLL:
     L.rosen_realspace_generate.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64,
                                            C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
     L.rosen_realspace_generate.restype = C.c_int
+    L.rosen_lattice_generate_async.argtypes = [i32, u64, u64, u64, C.POINTER(rosen_outputs), vp, vp]
+    L.rosen_lattice_generate_async.restype = C.c_int
+    L.rosen_realspace_generate_async.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64,
+                                                 C.POINTER(rosen_outputs), vp, vp]
+    L.rosen_realspace_generate_async.restype = C.c_int
     L.rosen_lattice_dump.argtypes = [i32, u64, u64, u64, vp, vp, i32, C.POINTER(rosen_summary), vp]
     L.rosen_lattice_dump.restype = C.c_int
     L.rosen_realspace_dump.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64, vp, vp, i32,
@@ -100,8 +105,10 @@ def _torch():
     return torch
 
 
-def _alloc_outputs(N: int, n_chains: int, conf_dtype: str, outputs: Iterable[str], device, host: bool):
-    """Allocate the requested per-chain buffers: torch CUDA tensors, or pinned host tensors."""
+def _alloc_outputs(N: int, n_chains: int, conf_dtype: str, outputs: Iterable[str], device, host: bool,
+                   cache: Optional[dict] = None):
+    """Allocate the requested per-chain buffers: torch CUDA tensors, or pinned host tensors.
+    `cache` (a dict the caller keeps) lets repeated calls reuse buffers of the same shape."""
     torch = _torch()
     want = set(outputs)
     unknown = want - set(PER_CHAIN)
@@ -114,7 +121,16 @@ def _alloc_outputs(N: int, n_chains: int, conf_dtype: str, outputs: Iterable[str
         "conf": ((n_chains, N, 3), torch.int32 if conf_dtype == "int32" else torch.float32),
         "ree2": ((n_chains,), torch.float64), "rg2": ((n_chains,), torch.float64),
     }
-    tensors = {k: torch.empty(shapes[k][0], dtype=shapes[k][1], **kw) for k in PER_CHAIN if k in want}
+    tensors = {}
+    for k in PER_CHAIN:
+        if k not in want:
+            continue
+        t = cache.get(k) if cache is not None else None
+        if t is None or tuple(t.shape) != shapes[k][0] or t.dtype != shapes[k][1] or t.is_cuda == host:
+            t = torch.empty(shapes[k][0], dtype=shapes[k][1], **kw)
+            if cache is not None:
+                cache[k] = t
+        tensors[k] = t
     st = rosen_outputs(*[tensors[k].data_ptr() if k in tensors else None for k in PER_CHAIN],
                        ROSEN_MEM_HOST if host else ROSEN_MEM_DEVICE, 0)
     return tensors, st
@@ -128,15 +144,15 @@ def _stream_ptr(stream) -> int:
 
 
 def rosen_lattice_generate(N: int, n_chains: int, seed: int, chain_offset: int = 0, outputs: Iterable[str] = (),
-                           summary: bool = True, stream=None, host_outputs: bool = False, device=None
-                           ) -> Tuple[Optional[Dict[str, float]], Dict[str, "object"]]:
+                           summary: bool = True, stream=None, host_outputs: bool = False, device=None,
+                           host_buffers: Optional[dict] = None) -> Tuple[Optional[Dict[str, float]], Dict[str, "object"]]:
     """rosen_lattice_generate of include/rosen.h. Returns (summary dict or None, {name: tensor})."""
     L = load_library()
     torch = _torch()
     device = device if device is not None else torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
     if device is None:
         raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
-    tensors, st = _alloc_outputs(N, n_chains, "int32", outputs, device, host_outputs)
+    tensors, st = _alloc_outputs(N, n_chains, "int32", outputs, device, host_outputs, host_buffers)
     s = rosen_summary()
     _check(L.rosen_lattice_generate(N, n_chains, seed, chain_offset, C.byref(st),
                                     C.byref(s) if summary else None, _stream_ptr(stream)))
@@ -145,7 +161,7 @@ def rosen_lattice_generate(N: int, n_chains: int, seed: int, chain_offset: int =
 
 def rosen_realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,
                              chain_offset: int = 0, outputs: Iterable[str] = (), summary: bool = True, stream=None,
-                             host_outputs: bool = False, device=None
+                             host_outputs: bool = False, device=None, host_buffers: Optional[dict] = None
                              ) -> Tuple[Optional[Dict[str, float]], Dict[str, "object"]]:
     """rosen_realspace_generate of include/rosen.h. Returns (summary dict or None, {name: tensor})."""
     L = load_library()
@@ -153,11 +169,46 @@ def rosen_realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: flo
     device = device if device is not None else torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
     if device is None:
         raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
-    tensors, st = _alloc_outputs(N, n_chains, "float32", outputs, device, host_outputs)
+    tensors, st = _alloc_outputs(N, n_chains, "float32", outputs, device, host_outputs, host_buffers)
     s = rosen_summary()
     _check(L.rosen_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, C.byref(st),
                                       C.byref(s) if summary else None, _stream_ptr(stream)))
     return (s.as_dict() if summary else None), tensors
+
+
+SUMMARY_BYTES = C.sizeof(rosen_summary)
+
+
+def _outputs_struct(tensors: Optional[Dict[str, "object"]]) -> rosen_outputs:
+    tensors = tensors or {}
+    return rosen_outputs(*[tensors[k].data_ptr() if k in tensors else None for k in PER_CHAIN], ROSEN_MEM_DEVICE, 0)
+
+
+def summary_from_device(summary_device) -> Dict[str, float]:
+    """Decode a uint8 CUDA tensor of SUMMARY_BYTES written by an _async call (synchronises via .cpu())."""
+    raw = bytes(summary_device.cpu().numpy().tobytes())
+    return rosen_summary.from_buffer_copy(raw).as_dict()
+
+
+def rosen_lattice_generate_async(N: int, n_chains: int, seed: int, chain_offset: int = 0, outputs=None,
+                                 summary_device=None, stream=None) -> None:
+    """rosen_lattice_generate_async: enqueue only. outputs = {name: CUDA tensor}; summary_device = uint8 CUDA
+    tensor of SUMMARY_BYTES (8-byte aligned) or None."""
+    L = load_library()
+    st = _outputs_struct(outputs)
+    _check(L.rosen_lattice_generate_async(N, n_chains, seed, chain_offset, C.byref(st),
+                                          summary_device.data_ptr() if summary_device is not None else None,
+                                          _stream_ptr(stream)))
+
+
+def rosen_realspace_generate_async(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,
+                                   chain_offset: int = 0, outputs=None, summary_device=None, stream=None) -> None:
+    """rosen_realspace_generate_async: enqueue only (see rosen_lattice_generate_async)."""
+    L = load_library()
+    st = _outputs_struct(outputs)
+    _check(L.rosen_realspace_generate_async(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, C.byref(st),
+                                            summary_device.data_ptr() if summary_device is not None else None,
+                                            _stream_ptr(stream)))
 
 
 def rosen_lattice_dump(N: int, n_chains: int, seed: int, chain_offset: int = 0, conf=None, lnW=None,

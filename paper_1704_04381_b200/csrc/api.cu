@@ -28,8 +28,9 @@ int fail_cuda(cudaError_t e, const char* what)
 
 // Per-device scratch: block partials + one total, and a pinned host mirror of the total.
 struct Scratch {
-    Partial* dev = nullptr;       // [kMaxPartials + 1]
-    Partial* host = nullptr;      // pinned, 1 element
+    Partial*       dev = nullptr;          // [kMaxPartials] block partials
+    rosen_summary* summary_dev = nullptr;  // written by finalize_kernel
+    rosen_summary* summary_host = nullptr; // pinned mirror
 };
 constexpr int kMaxDevices = 64;
 Scratch g_scratch[kMaxDevices];
@@ -43,8 +44,9 @@ int get_scratch(Scratch** out)
     std::lock_guard<std::mutex> lock(g_mutex);
     Scratch& s = g_scratch[dev];
     if (!s.dev) {
-        CK(cudaMalloc(&s.dev, sizeof(Partial) * (rosen::kMaxPartials + 1)));
-        CK(cudaMallocHost(&s.host, sizeof(Partial)));
+        CK(cudaMalloc(&s.dev, sizeof(Partial) * rosen::kMaxPartials));
+        CK(cudaMalloc(&s.summary_dev, sizeof(rosen_summary)));
+        CK(cudaMallocHost(&s.summary_host, sizeof(rosen_summary)));
     }
     *out = &s;
     return ROSEN_OK;
@@ -125,35 +127,27 @@ void derive(rosen_summary* s)
 }
 
 // After the generation kernel: second reduction pass, summary copy, host staging copies, sync.
+// summary (host) and summary_dev (device) are both optional; the finalize kernel runs if either is set.
 int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const rosen_outputs* outputs, const Sizes& z,
-           Staging& st, rosen_summary* summary, cudaStream_t stream)
+           Staging& st, rosen_summary* summary, rosen_summary* summary_dev, cudaStream_t stream)
 {
-    if (summary) {
-        if (rosen::launch_finalize(sc->dev, grid, sc->dev + rosen::kMaxPartials, stream) < 0) return fail_cuda(cudaGetLastError(), "finalize_kernel");
+    if (summary || summary_dev) {
+        rosen_summary* target = summary_dev ? summary_dev : sc->summary_dev;
+        if (rosen::launch_finalize(sc->dev, grid, n_chains, ln_shift, target, stream) < 0)
+            return fail_cuda(cudaGetLastError(), "finalize_kernel");
         ++g_launches;
-        CK(cudaMemcpyAsync(sc->host, sc->dev + rosen::kMaxPartials, sizeof(Partial), cudaMemcpyDeviceToHost, stream));
+        if (summary) CK(cudaMemcpyAsync(sc->summary_host, target, sizeof(rosen_summary), cudaMemcpyDeviceToHost, stream));
     }
     int rc = copy_back(outputs, z, st, stream);
     if (rc) return rc;
     st.release();
     if (summary || (outputs && outputs->memory == ROSEN_MEM_HOST)) CK(cudaStreamSynchronize(stream));
-    if (summary) {
-        const Partial& t = *sc->host;
-        summary->n_chains = n_chains; summary->n_dead = t.n_dead; summary->n_steps_attempted = t.n_steps;
-        summary->ln_shift = ln_shift;
-        summary->sum_w = t.sum_w; summary->sum_w_ree2 = t.sum_w_ree2; summary->sum_w_rg2 = t.sum_w_rg2; summary->sum_w2 = t.sum_w2;
-        summary->digest_xor = t.digest_xor; summary->digest_sum = t.digest_sum;
-        derive(summary);
-    }
+    if (summary) *summary = *sc->summary_host;
     return ROSEN_OK;
 }
 
-}  // namespace
-
-extern "C" {
-
-int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
-                           const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, const rosen_outputs* outputs,
+                 rosen_summary* summary, rosen_summary* summary_dev, void* cuda_stream)
 {
     g_err[0] = 0; g_launches = 0; g_kernel = "";
     if (N < 2 || n_chains == 0) { std::snprintf(g_err, sizeof(g_err), "need N >= 2 and n_chains >= 1"); return ROSEN_EINVAL; }
@@ -175,12 +169,12 @@ int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t
     rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");
     g_launches += rc;
-    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, stream);
+    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
 }
 
-int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
-                             uint64_t seed, uint64_t chain_offset,
-                             const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma, uint64_t seed,
+                   uint64_t chain_offset, const rosen_outputs* outputs, rosen_summary* summary,
+                   rosen_summary* summary_dev, void* cuda_stream)
 {
     g_err[0] = 0; g_launches = 0; g_kernel = "";
     if (N < 2 || n_chains == 0 || k_trials < 1 || k_trials > 255 || !(bond_len > 0.0f) || !(sigma >= 0.0f) ||
@@ -213,7 +207,43 @@ int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, flo
     rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space kernel launch");
     g_launches += rc;
-    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, stream);
+    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
+}
+
+}  // namespace
+
+extern "C" {
+
+int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                           const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    return lattice_impl(N, n_chains, seed, chain_offset, outputs, summary, nullptr, cuda_stream);
+}
+
+int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                             uint64_t seed, uint64_t chain_offset,
+                             const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    return realspace_impl(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, outputs, summary, nullptr, cuda_stream);
+}
+
+int rosen_lattice_generate_async(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                                 const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream)
+{
+    if (outputs && outputs->memory != ROSEN_MEM_DEVICE) {
+        std::snprintf(g_err, sizeof(g_err), "the _async calls take device outputs only"); return ROSEN_EINVAL;
+    }
+    return lattice_impl(N, n_chains, seed, chain_offset, outputs, nullptr, summary_device, cuda_stream);
+}
+
+int rosen_realspace_generate_async(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                                   uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream)
+{
+    if (outputs && outputs->memory != ROSEN_MEM_DEVICE) {
+        std::snprintf(g_err, sizeof(g_err), "the _async calls take device outputs only"); return ROSEN_EINVAL;
+    }
+    return realspace_impl(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, outputs, nullptr, summary_device, cuda_stream);
 }
 
 int rosen_lattice_dump(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
@@ -249,7 +279,7 @@ int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary
     return ROSEN_OK;
 }
 
-size_t rosen_workspace_bytes(void) { return sizeof(Partial) * (rosen::kMaxPartials + 1); }
+size_t rosen_workspace_bytes(void) { return sizeof(Partial) * rosen::kMaxPartials + sizeof(rosen_summary); }
 int32_t rosen_last_launch_count(void) { return g_launches; }
 const char* rosen_last_kernel_name(void) { return g_kernel; }
 

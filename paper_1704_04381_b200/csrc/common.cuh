@@ -50,6 +50,7 @@ constexpr int kMaxPartials = 4096;   // upper bound on gridDim.x of the generati
 // a negative ROSEN_E* code; *kernel_name receives a static string naming the variant chosen.
 int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
-int launch_finalize(const Partial* partials, int n_partials, Partial* total, cudaStream_t stream);
+int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift,
+                    void* summary_dev, cudaStream_t stream);   // summary_dev: rosen_summary* in device memory
 
 }  // namespace rosen

@@ -3,6 +3,7 @@
 // lives in shared memory as packed words split by monomer parity, because on a bipartite lattice
 // only monomers j with j = s (mod 2) can sit next to the growth point r_{s-1}: the scan of
 // Alg. 1 lines 13-17 / 26-31 touches floor(s/2) words instead of s-1 (exactly the same decisions).
+#include <algorithm>
 #include <math_constants.h>
 #include "common.cuh"
 #include "philox.cuh"
@@ -174,6 +175,8 @@ int launch_int(const LatticeParams& p, cudaStream_t stream, int* grid_out)
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    int smem_sm = 0;
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     const size_t fixed = sizeof(LatTables) + 8 * sizeof(Partial);
     const size_t per_thread = (size_t)stride_of(p.N) * 4;
     int threads = 256;
@@ -184,6 +187,10 @@ int launch_int(const LatticeParams& p, cudaStream_t stream, int* grid_out)
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
+    // The grid (hence the reduction tree) must not depend on the output variant: size it from the
+    // shared-memory / thread limits only, which are the same for every instantiation.
+    per_sm = (int)std::min<size_t>(2048 / threads, (size_t)(smem_sm - 1024) / (smem + 1024));
+    if (per_sm < 1) per_sm = 1;
     uint64_t want = (p.n_chains + threads - 1) / threads;
     uint64_t cap = (uint64_t)n_sm * per_sm;
     if (cap > (uint64_t)kMaxPartials) cap = kMaxPartials;

@@ -11,6 +11,7 @@
 //
 // All fp32 arithmetic that decides anything is written with explicit __f*_rn intrinsics in the order
 // DESIGN.md 3.3 fixes, so nvcc cannot contract or reorder it.
+#include <algorithm>
 #include <math_constants.h>
 #include "common.cuh"
 #include "philox.cuh"
@@ -249,6 +250,8 @@ int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    int smem_sm = 0;
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
     const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
     int threads = 256;
@@ -259,6 +262,9 @@ int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
+    // variant-independent grid (see lattice.cu): shared-memory / thread limits only
+    per_sm = (int)std::min<size_t>(2048 / threads, (size_t)(smem_sm - 1024) / (smem + 1024));
+    if (per_sm < 1) per_sm = 1;
     const uint64_t groups_per_block = threads / G;
     uint64_t want = (p.n_chains + groups_per_block - 1) / groups_per_block;
     uint64_t cap = (uint64_t)n_sm * per_sm;
