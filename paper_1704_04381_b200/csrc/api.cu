@@ -165,11 +165,12 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
     p.ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
     p.out = st.dev; p.partials = sc->dev;
+    rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks);
     int grid = 0;
     rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");
     g_launches += rc;
-    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
+    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
 }
 
 int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma, uint64_t seed,

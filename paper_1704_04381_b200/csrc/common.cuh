@@ -29,7 +29,9 @@ struct LatticeParams {
     uint32_t   key0, key1;      // Philox key = seed
     double     ln_shift;        // L
     DevOutputs out;
-    Partial*   partials;        // [gridDim.x]
+    Partial*   partials;        // [n_vblocks]
+    uint32_t   chunk;           // chains per virtual block (multiple of 256)
+    uint32_t   n_vblocks;       // ceil(n_chains / chunk) <= kMaxPartials
 };
 
 struct RealParams {
@@ -41,10 +43,26 @@ struct RealParams {
     float      b, sigma2, prefilter2;   // bond length, sigma^2 (fp32), conservative candidate radius^2
     double     ln_shift;
     DevOutputs out;
-    Partial*   partials;
+    Partial*   partials;        // [n_vblocks]
+    uint32_t   chunk;           // chains per virtual block (multiple of 256)
+    uint32_t   n_vblocks;
 };
 
-constexpr int kMaxPartials = 4096;   // upper bound on gridDim.x of the generation kernels
+// The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the
+// chain range [v*chunk, (v+1)*chunk) and produces partials[v] with a fixed thread mapping and tree, so
+// the sums depend on (n_chains, N) only -- never on the grid size, occupancy, output variant or GPU.
+constexpr int kMaxPartials = 8192;
+constexpr uint32_t kMinChunk = 2048;
+
+// chunk = chains per virtual block: >= kMinChunk, a multiple of 256, and large enough for <= kMaxPartials blocks.
+inline void partition_chains(uint64_t n_chains, uint32_t* chunk, uint32_t* n_vblocks)
+{
+    uint64_t c = (n_chains + kMaxPartials - 1) / kMaxPartials;
+    c = (c + 255) / 256 * 256;
+    if (c < kMinChunk) c = kMinChunk;
+    *chunk = (uint32_t)c;
+    *n_vblocks = (uint32_t)((n_chains + c - 1) / c);
+}
 
 // launchers (lattice.cu / realspace.cu / reduce.cu). Return the number of kernels launched or
 // a negative ROSEN_E* code; *kernel_name receives a static string naming the variant chosen.

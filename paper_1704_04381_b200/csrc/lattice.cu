@@ -1,8 +1,14 @@
 // lattice.cu -- cubic-lattice Rosenbluth chain generation for sm_100a (steps L0-L5 of DESIGN.md 2;
 // PAPER.md:88-179, Algorithm 1; weight Eq. 3 :58). One thread grows one chain at a time; the chain
-// lives in shared memory as packed words split by monomer parity, because on a bipartite lattice
-// only monomers j with j = s (mod 2) can sit next to the growth point r_{s-1}: the scan of
-// Alg. 1 lines 13-17 / 26-31 touches floor(s/2) words instead of s-1 (exactly the same decisions).
+// lives in shared memory as one packed key per monomer, split by monomer parity, because on a
+// bipartite lattice only monomers j with j = s (mod 2) can sit next to the growth point r_{s-1}: the
+// scan of Alg. 1 lines 13-17 / 26-31 touches floor(s/2) keys instead of s-1 (exactly the same decisions).
+//
+// The scan is the hot loop and is hand-scheduled in PTX: per 16-byte shared-memory
+// load (4 keys) it runs predicate-chained ISETP.EQ.OR compares -- one instruction per (key, neighbour)
+// pair, on the half-rate `alu` pipe -- and, for chains of N <= 128, moves the +-z neighbours to the
+// full-rate fp32 lanes: keys are stored as exactly representable floats, and prod_j (key_j - n_d) is zero
+// (or NaN after an overflow to inf) iff some key equals the neighbour key n_d. Both tests are exact.
 #include <algorithm>
 #include <math_constants.h>
 #include "common.cuh"
@@ -13,17 +19,20 @@ namespace rosen {
 
 namespace {
 
-// ---- packed site coordinates, 10-bit fields biased by 512 (|x| <= 511 => N <= 512) ------------------
-constexpr uint32_t kBias   = 512u;
-constexpr uint32_t kOrigin = kBias | (kBias << 10) | (kBias << 20);
-constexpr uint32_t kDX = 1u, kDY = 1u << 10, kDZ = 1u << 20;
+// ---- packed site keys ---------------------------------------------------------------------------
+// MIX  (N <= 128): 8-bit fields biased by 128, key < 2^24, stored as the fp32 number of that value.
+// !MIX (N <= 512): 10-bit fields biased by 512, stored as the integer itself.
+template <bool MIX> struct Key;
+template <> struct Key<true>  { static constexpr int kBits = 8,  kBias = 128; };
+template <> struct Key<false> { static constexpr int kBits = 10, kBias = 512; };
 
 struct LatTables {
     uint32_t lut[64];   // index = occupied-direction mask; bits 0-2 = m, bits 3+3i.. = i-th free direction
-    int4     step[8];   // per direction: {packed delta, dx, dy, dz}
+    int4     step[8];   // per direction: {key delta (float bits if MIX, else int), dx, dy, dz}
     double   ln_m[8];   // ln m; ln_m[0] = -inf (dead)
 };
 
+template <bool MIX>
 __device__ __forceinline__ void build_tables(LatTables* t)
 {
     for (int occ = threadIdx.x; occ < 64; occ += blockDim.x) {
@@ -37,7 +46,8 @@ __device__ __forceinline__ void build_tables(LatTables* t)
         const int ax = d >> 1, sg = (d & 1) ? -1 : 1;
         int4 s = make_int4(0, 0, 0, 0);
         if (d < 6) {
-            s.x = sg * (int)(1u << (10 * ax));
+            const int delta = sg * (1 << (Key<MIX>::kBits * ax));
+            s.x = MIX ? __float_as_int((float)delta) : delta;
             s.y = ax == 0 ? sg : 0; s.z = ax == 1 ? sg : 0; s.w = ax == 2 ? sg : 0;
         }
         t->step[d] = s;
@@ -51,154 +61,275 @@ __device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t
 }
 
 // stride (in 32-bit words) of one thread's chain storage: two parity arrays of half4 words each,
-// plus 4 words so that stride/4 is odd and LDS.128 of a quarter-warp is bank-conflict free.
+// plus 4 words so that stride/4 is odd (LDS.128 of a quarter-warp is bank-conflict free) and the
+// scan's one-chunk-ahead prefetch stays inside the thread's own region.
 __host__ __device__ inline int half4_of(int N) { return (((N + 1) / 2) + 3) & ~3; }
 __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 
-template <bool DIGEST, bool TRAJ>
-__global__ void __launch_bounds__(256) lattice_int_kernel(const LatticeParams p)
+// ---- L2: the scan ---------------------------------------------------------------------------------
+// addr: shared-memory byte address of the parity array; T >= 1 chunks of 4 keys; n0..n5: neighbour
+// keys in the order +x,-x,+y,-y,+z,-z. Returns the 6-bit mask of occupied neighbours. Unused slots
+// hold 0, which no neighbour key equals. Chunks are double-buffered (a*/b*) so that the next LDS.128
+// is in flight while the current 4 keys are tested.
+
+#define ROSEN_MIX_KEY(w)                                                                             \
+    "setp.eq.or.b32 p0, " #w ", %3, p0; setp.eq.or.b32 p1, " #w ", %4, p1;\n"                         \
+    "setp.eq.or.b32 p2, " #w ", %5, p2; setp.eq.or.b32 p3, " #w ", %6, p3;\n"
+#define ROSEN_MIX_FP(w, acc4, acc5)                                                                  \
+    "sub.rn.f32 t4, " #w ", %7; sub.rn.f32 t5, " #w ", %8;\n"                                         \
+    "mul.rn.f32 " #acc4 ", " #acc4 ", t4; mul.rn.f32 " #acc5 ", " #acc5 ", t5;\n"
+#define ROSEN_MIX_CHUNK(W)                                                                           \
+    ROSEN_MIX_KEY(W##0) ROSEN_MIX_FP(W##0, e4, e5) ROSEN_MIX_KEY(W##1) ROSEN_MIX_FP(W##1, f4, f5)     \
+    ROSEN_MIX_KEY(W##2) ROSEN_MIX_FP(W##2, e4, e5) ROSEN_MIX_KEY(W##3) ROSEN_MIX_FP(W##3, f4, f5)
+
+__device__ __forceinline__ uint32_t scan_mix(uint32_t addr, uint32_t T, uint32_t n0, uint32_t n1, uint32_t n2,
+                                             uint32_t n3, uint32_t n4, uint32_t n5)
+{
+    uint32_t occ;
+    asm volatile("{\n"
+        ".reg .pred p0, p1, p2, p3, q;\n"
+        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, r0, r1, r2, r3, r4, r5;\n"
+        ".reg .f32 e4, e5, f4, f5, t4, t5;\n"
+        "mov.u32 ad, %1; mov.u32 cnt, %2;\n"
+        "setp.lt.u32 p0, cnt, 0; setp.lt.u32 p1, cnt, 0; setp.lt.u32 p2, cnt, 0; setp.lt.u32 p3, cnt, 0;\n"
+        "mov.f32 e4, 0f3F800000; mov.f32 e5, 0f3F800000; mov.f32 f4, 0f3F800000; mov.f32 f5, 0f3F800000;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
+        "SCAN_LOOP:\n"
+        "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
+        ROSEN_MIX_CHUNK(a)
+        "setp.eq.u32 q, cnt, 1;\n"
+        "@q bra SCAN_DONE;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
+        ROSEN_MIX_CHUNK(b)
+        "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
+        "setp.ne.u32 q, cnt, 0;\n"
+        "@q bra SCAN_LOOP;\n"
+        "SCAN_DONE:\n"
+        "mul.rn.f32 e4, e4, f4; mul.rn.f32 e5, e5, f5;\n"
+        "selp.u32 r0, 1, 0, p0; selp.u32 r1, 2, 0, p1; selp.u32 r2, 4, 0, p2; selp.u32 r3, 8, 0, p3;\n"
+        "setp.equ.f32 p0, e4, 0f00000000; setp.equ.f32 p1, e5, 0f00000000;\n"   // zero, or NaN = inf * 0
+        "selp.u32 r4, 16, 0, p0; selp.u32 r5, 32, 0, p1;\n"
+        "add.u32 r0, r0, r1; add.u32 r2, r2, r3; add.u32 r4, r4, r5;\n"
+        "add.u32 r0, r0, r2; add.u32 %0, r0, r4;\n"
+        "}\n"
+        : "=r"(occ)
+        : "r"(addr), "r"(T), "r"(n0), "r"(n1), "r"(n2), "r"(n3), "r"(n4), "r"(n5)
+        : "memory");
+    return occ;
+}
+
+#define ROSEN_INT_KEY(w)                                                                             \
+    "setp.eq.or.b32 p0, " #w ", %3, p0; setp.eq.or.b32 p1, " #w ", %4, p1; setp.eq.or.b32 p2, " #w ", %5, p2;\n" \
+    "setp.eq.or.b32 p3, " #w ", %6, p3; setp.eq.or.b32 p4, " #w ", %7, p4; setp.eq.or.b32 p5, " #w ", %8, p5;\n"
+#define ROSEN_INT_CHUNK(W) ROSEN_INT_KEY(W##0) ROSEN_INT_KEY(W##1) ROSEN_INT_KEY(W##2) ROSEN_INT_KEY(W##3)
+
+__device__ __forceinline__ uint32_t scan_int(uint32_t addr, uint32_t T, uint32_t n0, uint32_t n1, uint32_t n2,
+                                             uint32_t n3, uint32_t n4, uint32_t n5)
+{
+    uint32_t occ;
+    asm volatile("{\n"
+        ".reg .pred p0, p1, p2, p3, p4, p5, q;\n"
+        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, r0, r1, r2, r3, r4, r5;\n"
+        "mov.u32 ad, %1; mov.u32 cnt, %2;\n"
+        "setp.lt.u32 p0, cnt, 0; setp.lt.u32 p1, cnt, 0; setp.lt.u32 p2, cnt, 0;\n"
+        "setp.lt.u32 p3, cnt, 0; setp.lt.u32 p4, cnt, 0; setp.lt.u32 p5, cnt, 0;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
+        "SCAN_LOOP:\n"
+        "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
+        ROSEN_INT_CHUNK(a)
+        "setp.eq.u32 q, cnt, 1;\n"
+        "@q bra SCAN_DONE;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
+        ROSEN_INT_CHUNK(b)
+        "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
+        "setp.ne.u32 q, cnt, 0;\n"
+        "@q bra SCAN_LOOP;\n"
+        "SCAN_DONE:\n"
+        "selp.u32 r0, 1, 0, p0; selp.u32 r1, 2, 0, p1; selp.u32 r2, 4, 0, p2;\n"
+        "selp.u32 r3, 8, 0, p3; selp.u32 r4, 16, 0, p4; selp.u32 r5, 32, 0, p5;\n"
+        "add.u32 r0, r0, r1; add.u32 r2, r2, r3; add.u32 r4, r4, r5;\n"
+        "add.u32 r0, r0, r2; add.u32 %0, r0, r4;\n"
+        "}\n"
+        : "=r"(occ)
+        : "r"(addr), "r"(T), "r"(n0), "r"(n1), "r"(n2), "r"(n3), "r"(n4), "r"(n5)
+        : "memory");
+    return occ;
+}
+
+template <bool MIX>
+__device__ __forceinline__ uint32_t key_add(uint32_t h, int delta_key)
+{
+    return MIX ? __float_as_uint(__fadd_rn(__uint_as_float(h), __int_as_float(delta_key))) : h + (uint32_t)delta_key;
+}
+
+// key delta of +1 along axis ax, in the key's own encoding
+template <bool MIX>
+__device__ __forceinline__ constexpr int unit_delta(int ax)
+{
+    return 1 << (Key<MIX>::kBits * ax);
+}
+
+template <bool MIX, bool DIGEST, bool TRAJ>
+__global__ void __launch_bounds__(256) lattice_kernel(const LatticeParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     LatTables* tab = reinterpret_cast<LatTables*>(smem_raw);
     Partial* scratch = reinterpret_cast<Partial*>(smem_raw + sizeof(LatTables));
     uint32_t* chains = reinterpret_cast<uint32_t*>(smem_raw + sizeof(LatTables) + 8 * sizeof(Partial));
 
+    constexpr int kBits = Key<MIX>::kBits, kBias = Key<MIX>::kBias;
+    constexpr uint32_t kFieldMask = (1u << kBits) - 1u;
+    constexpr uint32_t kOriginInt = (uint32_t)kBias | ((uint32_t)kBias << kBits) | ((uint32_t)kBias << (2 * kBits));
+    const uint32_t kOrigin = MIX ? __float_as_uint((float)kOriginInt) : kOriginInt;
+    // neighbour key offsets (compile-time constants in the key's encoding)
+    const uint32_t dxp = MIX ? __float_as_uint(1.0f) : 1u;
+    (void)dxp;
+
     const int N = p.N;
     const int half4 = half4_of(N), stride = stride_of(N);
     uint32_t* ev = chains + (size_t)threadIdx.x * stride;   // monomers 0,2,4,...
     uint32_t* od = ev + half4;                              // monomers 1,3,5,...
+    const uint32_t ev_addr = (uint32_t)__cvta_generic_to_shared(ev);
+    const uint32_t od_addr = ev_addr + (uint32_t)half4 * 4u;
 
-    build_tables(tab);
+    build_tables<MIX>(tab);
     __syncthreads();
 
-    Partial acc = partial_zero();
-    const uint64_t nthreads = (uint64_t)gridDim.x * blockDim.x;
+    const uint32_t per_thread = p.chunk / blockDim.x;       // chunk is a multiple of 256 >= blockDim.x
 
-    for (uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < p.n_chains; idx += nthreads) {
-        const uint64_t chain = p.chain_offset + idx;
-        const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
+    for (uint32_t vb = blockIdx.x; vb < p.n_vblocks; vb += gridDim.x) {
+        Partial acc = partial_zero();
+        for (uint32_t it = 0; it < per_thread; ++it) {
+            const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * blockDim.x + threadIdx.x;
+            if (idx >= p.n_chains) break;
+            const uint64_t chain = p.chain_offset + idx;
+            const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
 
-        // L0: r_0 = origin, lnW = 0, alive. Unused words hold 0, which no neighbour word can equal.
-        for (int i = 0; i < stride / 4; ++i) reinterpret_cast<uint4*>(ev)[i] = make_uint4(0, 0, 0, 0);
-        ev[0] = kOrigin;
-        uint32_t h = kOrigin;
-        int hx = 0, hy = 0, hz = 0, sx = 0, sy = 0, sz = 0, s2 = 0;
-        double lnW = 0.0;
-        bool alive = true;
-        uint32_t steps = 0;
-        uint64_t dg = 0xCBF29CE484222325ull;
-        uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
+            // L0: r_0 = origin, lnW = 0, alive. Unused words hold 0, which no neighbour key can equal.
+            for (int i = 0; i < stride / 4; ++i) reinterpret_cast<uint4*>(ev)[i] = make_uint4(0, 0, 0, 0);
+            ev[0] = kOrigin;
+            uint32_t h = kOrigin;
+            int hx = 0, hy = 0, hz = 0, sx = 0, sy = 0, sz = 0, s2 = 0;
+            double lnW = 0.0;
+            bool alive = true;
+            uint32_t steps = 0;
+            uint64_t dg = 0xCBF29CE484222325ull;
+            uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
 
-        for (int q = 0; 4 * q < N; ++q) {
-            uint32_t w[4];
-            philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.key0, p.key1, w);   // L1: one block per 4 steps
+            for (int q = 0; 4 * q < N; ++q) {
+                uint32_t w[4];
+                philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.key0, p.key1, w);   // L1: one block per 4 steps
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int s = 4 * q + k;
-                if (s == 0 || s >= N) continue;
+                for (int k = 0; k < 4; ++k) {
+                    const int s = 4 * q + k;
+                    if (s == 0 || s >= N) continue;
 
-                // L2: which of the 6 neighbours of r_{s-1} are occupied by r_j, j = s-2, s-4, ...
-                const uint32_t n0 = h + kDX, n1 = h - kDX, n2 = h + kDY, n3 = h - kDY, n4 = h + kDZ, n5 = h - kDZ;
-                bool o0 = false, o1 = false, o2 = false, o3 = false, o4 = false, o5 = false;
-                const uint4* A = reinterpret_cast<const uint4*>((s & 1) ? od : ev);
-                const int iters = ((s >> 1) + 3) >> 2;
-                for (int i = 0; i < iters; ++i) {
-                    const uint4 v = A[i];
-                    o0 |= (v.x == n0); o1 |= (v.x == n1); o2 |= (v.x == n2); o3 |= (v.x == n3); o4 |= (v.x == n4); o5 |= (v.x == n5);
-                    o0 |= (v.y == n0); o1 |= (v.y == n1); o2 |= (v.y == n2); o3 |= (v.y == n3); o4 |= (v.y == n4); o5 |= (v.y == n5);
-                    o0 |= (v.z == n0); o1 |= (v.z == n1); o2 |= (v.z == n2); o3 |= (v.z == n3); o4 |= (v.z == n4); o5 |= (v.z == n5);
-                    o0 |= (v.w == n0); o1 |= (v.w == n1); o2 |= (v.w == n2); o3 |= (v.w == n3); o4 |= (v.w == n4); o5 |= (v.w == n5);
+                    // L2: which of the 6 neighbours of r_{s-1} are occupied by r_j, j = s-2, s-4, ...
+                    uint32_t occ = 0;
+                    const uint32_t T = (uint32_t)(((s >> 1) + 3) >> 2);
+                    if (T != 0u) {
+                        const uint32_t n0 = key_add<MIX>(h, MIX ? __float_as_int(1.0f) : 1);
+                        const uint32_t n1 = key_add<MIX>(h, MIX ? __float_as_int(-1.0f) : -1);
+                        const uint32_t n2 = key_add<MIX>(h, MIX ? __float_as_int((float)(1 << kBits)) : (1 << kBits));
+                        const uint32_t n3 = key_add<MIX>(h, MIX ? __float_as_int(-(float)(1 << kBits)) : -(1 << kBits));
+                        const uint32_t n4 = key_add<MIX>(h, MIX ? __float_as_int((float)(1 << (2 * kBits))) : (1 << (2 * kBits)));
+                        const uint32_t n5 = key_add<MIX>(h, MIX ? __float_as_int(-(float)(1 << (2 * kBits))) : -(1 << (2 * kBits)));
+                        const uint32_t addr = (k & 1) ? od_addr : ev_addr;
+                        occ = MIX ? scan_mix(addr, T, n0, n1, n2, n3, n4, n5) : scan_int(addr, T, n0, n1, n2, n3, n4, n5);
+                    }
+                    const uint32_t e = tab->lut[occ];
+                    const uint32_t m = e & 7u;
+
+                    // L3: weight. ln_m[0] = -inf makes a dead chain's lnW -inf for good.
+                    steps += alive ? 1u : 0u;
+                    lnW += tab->ln_m[m];
+                    if (TRAJ && mrow) mrow[s - 1] = alive ? (uint8_t)m : (uint8_t)0;
+
+                    // L4: uniform choice among the free neighbours, then place monomer s
+                    const uint32_t sel = __umulhi(w[k], m);
+                    const uint32_t dir = (e >> (3u + 3u * sel)) & 7u;
+                    if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? dir : 0xFFu); }
+                    alive = alive && (m != 0u);
+                    const int4 st = tab->step[dir];
+                    h = key_add<MIX>(h, st.x); hx += st.y; hy += st.z; hz += st.w;
+                    ((k & 1) ? od : ev)[s >> 1] = h;
+
+                    // L5: running sums for Rg^2
+                    sx += hx; sy += hy; sz += hz; s2 += hx * hx + hy * hy + hz * hz;
                 }
-                const uint32_t occ = (uint32_t)o0 | ((uint32_t)o1 << 1) | ((uint32_t)o2 << 2) | ((uint32_t)o3 << 3) |
-                                     ((uint32_t)o4 << 4) | ((uint32_t)o5 << 5);
-                const uint32_t e = tab->lut[occ];
-                const uint32_t m = e & 7u;
+            }
 
-                // L3: weight. ln_m[0] = -inf makes a dead chain's lnW -inf for good.
-                steps += alive ? 1u : 0u;
-                lnW += tab->ln_m[m];
-                if (TRAJ && mrow) mrow[s - 1] = alive ? (uint8_t)m : (uint8_t)0;
+            // L5: per-chain observables (integers until the final divide)
+            double ree2 = 0.0, rg2 = 0.0;
+            if (alive) {
+                ree2 = (double)(hx * hx + hy * hy + hz * hz);
+                const long long num = (long long)N * s2 - ((long long)sx * sx + (long long)sy * sy + (long long)sz * sz);
+                rg2 = (double)num / ((double)N * (double)N);
+            }
+            const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
+            acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
+            acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
+            if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
 
-                // L4: uniform choice among the free neighbours, then place monomer s
-                const uint32_t sel = __umulhi(w[k], m);
-                const uint32_t dir = (e >> (3u + 3u * sel)) & 7u;
-                if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? dir : 0xFFu); }
-                alive = alive && (m != 0u);
-                const int4 st = tab->step[dir];
-                h += (uint32_t)st.x; hx += st.y; hy += st.z; hz += st.w;
-                ((s & 1) ? od : ev)[s >> 1] = h;
-
-                // L5: running sums for Rg^2
-                sx += hx; sy += hy; sz += hz; s2 += hx * hx + hy * hy + hz * hz;
+            if (p.out.lnW) p.out.lnW[idx] = lnW;
+            if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
+            if (p.out.ree2) p.out.ree2[idx] = ree2;
+            if (p.out.rg2) p.out.rg2[idx] = rg2;
+            if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
+            if (TRAJ && p.out.conf) {
+                // D1 (lattice): each thread unpacks and writes its own chain; monomers from the death
+                // step on are zero. steps = death step for a dead chain.
+                int32_t* c = reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3;
+                const int placed = alive ? N : (int)steps;
+                for (int i = 0; i < N; ++i) {
+                    const uint32_t raw = ((i & 1) ? od : ev)[i >> 1];
+                    const uint32_t v = MIX ? (uint32_t)__float2int_rn(__uint_as_float(raw)) : raw;
+                    const bool ok = i < placed;
+                    c[3 * i + 0] = ok ? (int)(v & kFieldMask) - kBias : 0;
+                    c[3 * i + 1] = ok ? (int)((v >> kBits) & kFieldMask) - kBias : 0;
+                    c[3 * i + 2] = ok ? (int)((v >> (2 * kBits)) & kFieldMask) - kBias : 0;
+                }
             }
         }
-
-        // L5: per-chain observables (integers until the final divide)
-        double ree2 = 0.0, rg2 = 0.0;
-        if (alive) {
-            ree2 = (double)(hx * hx + hy * hy + hz * hz);
-            const long long num = (long long)N * s2 - ((long long)sx * sx + (long long)sy * sy + (long long)sz * sz);
-            rg2 = (double)num / ((double)N * (double)N);
-        }
-        const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
-        acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
-        acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
-        if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
-
-        if (p.out.lnW) p.out.lnW[idx] = lnW;
-        if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
-        if (p.out.ree2) p.out.ree2[idx] = ree2;
-        if (p.out.rg2) p.out.rg2[idx] = rg2;
-        if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
-        if (TRAJ && p.out.conf) {
-            // D1 (first version): each thread unpacks and writes its own chain; monomers from the
-            // death step on are zero. steps = death step for a dead chain.
-            int32_t* c = reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3;
-            const int placed = alive ? N : (int)steps;
-            for (int i = 0; i < N; ++i) {
-                const uint32_t v = ((i & 1) ? od : ev)[i >> 1];
-                const bool ok = i < placed;
-                c[3 * i + 0] = ok ? (int)(v & 1023u) - (int)kBias : 0;
-                c[3 * i + 1] = ok ? (int)((v >> 10) & 1023u) - (int)kBias : 0;
-                c[3 * i + 2] = ok ? (int)((v >> 20) & 1023u) - (int)kBias : 0;
-            }
-        }
+        block_reduce_store(acc, scratch, p.partials + vb);
     }
-
-    block_reduce_store(acc, scratch, p.partials + blockIdx.x);
 }
 
-template <bool DIGEST, bool TRAJ>
-int launch_int(const LatticeParams& p, cudaStream_t stream, int* grid_out)
+template <bool MIX, bool DIGEST, bool TRAJ>
+int launch_variant(const LatticeParams& p, cudaStream_t stream, int* grid_out)
 {
     int dev = 0, n_sm = 0, smem_max = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    int smem_sm = 0;
-    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     const size_t fixed = sizeof(LatTables) + 8 * sizeof(Partial);
     const size_t per_thread = (size_t)stride_of(p.N) * 4;
+    // threads per block depends on N only (never on the output variant): it fixes the reduction tree.
     int threads = 256;
     while (threads > 32 && fixed + per_thread * threads > (size_t)(72 * 1024)) threads >>= 1;
     const size_t smem = fixed + per_thread * threads;
     if (smem > (size_t)smem_max) return -2;
-    auto kern = lattice_int_kernel<DIGEST, TRAJ>;
+    auto kern = lattice_kernel<MIX, DIGEST, TRAJ>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
-    // The grid (hence the reduction tree) must not depend on the output variant: size it from the
-    // shared-memory / thread limits only, which are the same for every instantiation.
-    per_sm = (int)std::min<size_t>(2048 / threads, (size_t)(smem_sm - 1024) / (smem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    uint64_t want = (p.n_chains + threads - 1) / threads;
-    uint64_t cap = (uint64_t)n_sm * per_sm;
-    if (cap > (uint64_t)kMaxPartials) cap = kMaxPartials;
-    const int grid = (int)(want < cap ? want : cap);
+    // One resident wave; virtual blocks (common.cuh) are strided over it, so the grid is free to follow
+    // the real occupancy of this variant without touching the sums.
+    const uint32_t cap = (uint32_t)n_sm * (uint32_t)per_sm;
+    const int grid = (int)(p.n_vblocks < cap ? p.n_vblocks : cap);
     kern<<<grid, threads, smem, stream>>>(p);
     if (cudaGetLastError() != cudaSuccess) return -3;
     *grid_out = grid;
     return 1;
+}
+
+template <bool MIX>
+int launch_mix(const LatticeParams& p, cudaStream_t stream, int* grid_out)
+{
+    const bool digest = p.out.digest != nullptr;
+    const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
+    if (traj) return digest ? launch_variant<MIX, true, true>(p, stream, grid_out) : launch_variant<MIX, false, true>(p, stream, grid_out);
+    return digest ? launch_variant<MIX, true, false>(p, stream, grid_out) : launch_variant<MIX, false, false>(p, stream, grid_out);
 }
 
 }  // namespace
@@ -207,12 +338,14 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
 {
     const bool digest = p.out.digest != nullptr;
     const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
-    if (traj) {
-        *kernel_name = digest ? "lattice_int_kernel<digest,traj>" : "lattice_int_kernel<traj>";
-        return digest ? launch_int<true, true>(p, stream, grid_out) : launch_int<false, true>(p, stream, grid_out);
+    if (p.N <= 128) {   // keys < 2^24 are exact in fp32: mixed ISETP / fp32-product scan
+        *kernel_name = traj ? (digest ? "lattice_kernel<mix,digest,traj>" : "lattice_kernel<mix,traj>")
+                            : (digest ? "lattice_kernel<mix,digest>" : "lattice_kernel<mix>");
+        return launch_mix<true>(p, stream, grid_out);
     }
-    *kernel_name = digest ? "lattice_int_kernel<digest>" : "lattice_int_kernel<>";
-    return digest ? launch_int<true, false>(p, stream, grid_out) : launch_int<false, false>(p, stream, grid_out);
+    *kernel_name = traj ? (digest ? "lattice_kernel<int,digest,traj>" : "lattice_kernel<int,traj>")
+                        : (digest ? "lattice_kernel<int,digest>" : "lattice_kernel<int>");
+    return launch_mix<false>(p, stream, grid_out);
 }
 
 }  // namespace rosen
