@@ -27,7 +27,9 @@ template <> struct Key<true>  { static constexpr int kBits = 8,  kBias = 128; };
 template <> struct Key<false> { static constexpr int kBits = 10, kBias = 512; };
 
 struct LatTables {
-    uint32_t lut[64];   // index = occupied-direction mask; bits 0-2 = m, bits 3+3i.. = i-th free direction
+    uint2    lut[64];   // index = occupied-direction mask. .x: bits 0-2 = m, bits 4+4i..6+4i = i-th free direction
+                        // (so that (x >> 4*sel) & 0x70 is the byte offset of step[dir]); .y: histogram increment
+                        // 1 << 8*(m-2) for m = 2..5, else 0 (m = 1 adds ln 1 = 0, m = 6 happens at s = 1 only)
     int4     step[8];   // per direction: {key delta (float bits if MIX, else int), dx, dy, dz}
     double   ln_m[8];   // ln m; ln_m[0] = -inf (dead)
 };
@@ -38,8 +40,8 @@ __device__ __forceinline__ void build_tables(LatTables* t)
     for (int occ = threadIdx.x; occ < 64; occ += blockDim.x) {
         uint32_t e = 0, m = 0;
         for (int d = 0; d < 6; ++d)
-            if (!((occ >> d) & 1)) { e |= (uint32_t)d << (3 + 3 * m); ++m; }
-        t->lut[occ] = e | m;
+            if (!((occ >> d) & 1)) { e |= (uint32_t)d << (4 + 4 * m); ++m; }
+        t->lut[occ] = make_uint2(e | m, (m >= 2 && m <= 5) ? 1u << (8 * (m - 2)) : 0u);
     }
     if (threadIdx.x < 8) {
         const int d = threadIdx.x;
@@ -70,8 +72,9 @@ __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 // addr: shared-memory byte address of the parity array; T >= 1 chunks of 4 keys; n0..n5: neighbour
 // keys in the order +x,-x,+y,-y,+z,-z. Returns the 6-bit mask of occupied neighbours. Unused slots
 // hold 0, which no neighbour key equals. Chunks are double-buffered (a*/b*) so that the next LDS.128
-// is in flight while the current 4 keys are tested.
-
+// is in flight while the current 4 keys are tested; the first chunk is peeled so that it initialises
+// the predicate chains and the fp32 products instead of separate set-up instructions. The loads run
+// at most one chunk past the T-th, which stays inside the thread's own region (stride_of).
 #define ROSEN_MIX_KEY(w)                                                                             \
     "setp.eq.or.b32 p0, " #w ", %3, p0; setp.eq.or.b32 p1, " #w ", %4, p1;\n"                         \
     "setp.eq.or.b32 p2, " #w ", %5, p2; setp.eq.or.b32 p3, " #w ", %6, p3;\n"
@@ -81,6 +84,10 @@ __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 #define ROSEN_MIX_CHUNK(W)                                                                           \
     ROSEN_MIX_KEY(W##0) ROSEN_MIX_FP(W##0, e4, e5) ROSEN_MIX_KEY(W##1) ROSEN_MIX_FP(W##1, f4, f5)     \
     ROSEN_MIX_KEY(W##2) ROSEN_MIX_FP(W##2, e4, e5) ROSEN_MIX_KEY(W##3) ROSEN_MIX_FP(W##3, f4, f5)
+#define ROSEN_MIX_FIRST(W)                                                                           \
+    "setp.eq.b32 p0, " #W "0, %3; setp.eq.b32 p1, " #W "0, %4; setp.eq.b32 p2, " #W "0, %5; setp.eq.b32 p3, " #W "0, %6;\n" \
+    "sub.rn.f32 e4, " #W "0, %7; sub.rn.f32 e5, " #W "0, %8; sub.rn.f32 f4, " #W "1, %7; sub.rn.f32 f5, " #W "1, %8;\n"     \
+    ROSEN_MIX_KEY(W##1) ROSEN_MIX_KEY(W##2) ROSEN_MIX_FP(W##2, e4, e5) ROSEN_MIX_KEY(W##3) ROSEN_MIX_FP(W##3, f4, f5)
 
 __device__ __forceinline__ uint32_t scan_mix(uint32_t addr, uint32_t T, uint32_t n0, uint32_t n1, uint32_t n2,
                                              uint32_t n3, uint32_t n4, uint32_t n5)
@@ -91,18 +98,20 @@ __device__ __forceinline__ uint32_t scan_mix(uint32_t addr, uint32_t T, uint32_t
         ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, r0, r1, r2, r3, r4, r5;\n"
         ".reg .f32 e4, e5, f4, f5, t4, t5;\n"
         "mov.u32 ad, %1; mov.u32 cnt, %2;\n"
-        "setp.lt.u32 p0, cnt, 0; setp.lt.u32 p1, cnt, 0; setp.lt.u32 p2, cnt, 0; setp.lt.u32 p3, cnt, 0;\n"
-        "mov.f32 e4, 0f3F800000; mov.f32 e5, 0f3F800000; mov.f32 f4, 0f3F800000; mov.f32 f5, 0f3F800000;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
-        "SCAN_LOOP:\n"
         "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
-        ROSEN_MIX_CHUNK(a)
+        ROSEN_MIX_FIRST(a)
         "setp.eq.u32 q, cnt, 1;\n"
         "@q bra SCAN_DONE;\n"
+        "SCAN_LOOP:\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
         ROSEN_MIX_CHUNK(b)
+        "setp.eq.u32 q, cnt, 2;\n"
+        "@q bra SCAN_DONE;\n"
+        "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+48];\n"
+        ROSEN_MIX_CHUNK(a)
         "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
-        "setp.ne.u32 q, cnt, 0;\n"
+        "setp.ne.u32 q, cnt, 1;\n"
         "@q bra SCAN_LOOP;\n"
         "SCAN_DONE:\n"
         "mul.rn.f32 e4, e4, f4; mul.rn.f32 e5, e5, f5;\n"
@@ -122,6 +131,10 @@ __device__ __forceinline__ uint32_t scan_mix(uint32_t addr, uint32_t T, uint32_t
     "setp.eq.or.b32 p0, " #w ", %3, p0; setp.eq.or.b32 p1, " #w ", %4, p1; setp.eq.or.b32 p2, " #w ", %5, p2;\n" \
     "setp.eq.or.b32 p3, " #w ", %6, p3; setp.eq.or.b32 p4, " #w ", %7, p4; setp.eq.or.b32 p5, " #w ", %8, p5;\n"
 #define ROSEN_INT_CHUNK(W) ROSEN_INT_KEY(W##0) ROSEN_INT_KEY(W##1) ROSEN_INT_KEY(W##2) ROSEN_INT_KEY(W##3)
+#define ROSEN_INT_FIRST(W)                                                                           \
+    "setp.eq.b32 p0, " #W "0, %3; setp.eq.b32 p1, " #W "0, %4; setp.eq.b32 p2, " #W "0, %5;\n"        \
+    "setp.eq.b32 p3, " #W "0, %6; setp.eq.b32 p4, " #W "0, %7; setp.eq.b32 p5, " #W "0, %8;\n"        \
+    ROSEN_INT_KEY(W##1) ROSEN_INT_KEY(W##2) ROSEN_INT_KEY(W##3)
 
 __device__ __forceinline__ uint32_t scan_int(uint32_t addr, uint32_t T, uint32_t n0, uint32_t n1, uint32_t n2,
                                              uint32_t n3, uint32_t n4, uint32_t n5)
@@ -131,18 +144,20 @@ __device__ __forceinline__ uint32_t scan_int(uint32_t addr, uint32_t T, uint32_t
         ".reg .pred p0, p1, p2, p3, p4, p5, q;\n"
         ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, r0, r1, r2, r3, r4, r5;\n"
         "mov.u32 ad, %1; mov.u32 cnt, %2;\n"
-        "setp.lt.u32 p0, cnt, 0; setp.lt.u32 p1, cnt, 0; setp.lt.u32 p2, cnt, 0;\n"
-        "setp.lt.u32 p3, cnt, 0; setp.lt.u32 p4, cnt, 0; setp.lt.u32 p5, cnt, 0;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
-        "SCAN_LOOP:\n"
         "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
-        ROSEN_INT_CHUNK(a)
+        ROSEN_INT_FIRST(a)
         "setp.eq.u32 q, cnt, 1;\n"
         "@q bra SCAN_DONE;\n"
+        "SCAN_LOOP:\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
         ROSEN_INT_CHUNK(b)
+        "setp.eq.u32 q, cnt, 2;\n"
+        "@q bra SCAN_DONE;\n"
+        "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+48];\n"
+        ROSEN_INT_CHUNK(a)
         "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
-        "setp.ne.u32 q, cnt, 0;\n"
+        "setp.ne.u32 q, cnt, 1;\n"
         "@q bra SCAN_LOOP;\n"
         "SCAN_DONE:\n"
         "selp.u32 r0, 1, 0, p0; selp.u32 r1, 2, 0, p1; selp.u32 r2, 4, 0, p2;\n"
@@ -211,7 +226,8 @@ __global__ void __launch_bounds__(256) lattice_kernel(const LatticeParams p)
             uint32_t h = kOrigin;
             int hx = 0, hy = 0, hz = 0, sx = 0, sy = 0, sz = 0, s2 = 0;
             double lnW = 0.0;
-            bool alive = true;
+            uint32_t hist = 0;                 // MIX: counts of m = 2,3,4,5 in bytes 0..3
+            uint32_t alive_i = 1u;
             uint32_t steps = 0;
             uint64_t dg = 0xCBF29CE484222325ull;
             uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
@@ -237,20 +253,22 @@ __global__ void __launch_bounds__(256) lattice_kernel(const LatticeParams p)
                         const uint32_t addr = (k & 1) ? od_addr : ev_addr;
                         occ = MIX ? scan_mix(addr, T, n0, n1, n2, n3, n4, n5) : scan_int(addr, T, n0, n1, n2, n3, n4, n5);
                     }
-                    const uint32_t e = tab->lut[occ];
+                    const uint2 le = tab->lut[occ];
+                    const uint32_t e = le.x;
                     const uint32_t m = e & 7u;
 
-                    // L3: weight. ln_m[0] = -inf makes a dead chain's lnW -inf for good.
-                    steps += alive ? 1u : 0u;
-                    lnW += tab->ln_m[m];
-                    if (TRAJ && mrow) mrow[s - 1] = alive ? (uint8_t)m : (uint8_t)0;
+                    // L3: weight. MIX: histogram of m (packed 8-bit counts, N <= 128), lnW assembled once per
+                    // chain; else lnW += ln m with ln_m[0] = -inf. alive_i = 1 until the first m = 0.
+                    steps += alive_i;
+                    if (MIX) hist += le.y; else lnW += tab->ln_m[m];
+                    if (TRAJ && mrow) mrow[s - 1] = alive_i ? (uint8_t)m : (uint8_t)0;
 
                     // L4: uniform choice among the free neighbours, then place monomer s
                     const uint32_t sel = __umulhi(w[k], m);
-                    const uint32_t dir = (e >> (3u + 3u * sel)) & 7u;
-                    if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? dir : 0xFFu); }
-                    alive = alive && (m != 0u);
-                    const int4 st = tab->step[dir];
+                    const uint32_t off = (e >> (4u * sel)) & 0x70u;          // 16 * direction
+                    if (DIGEST) { if (alive_i) dg = digest_fold(dg, m, m ? (off >> 4) : 0xFFu); }
+                    alive_i &= min(m, 1u);
+                    const int4 st = *reinterpret_cast<const int4*>(reinterpret_cast<const unsigned char*>(tab->step) + off);
                     h = key_add<MIX>(h, st.x); hx += st.y; hy += st.z; hz += st.w;
                     ((k & 1) ? od : ev)[s >> 1] = h;
 
@@ -260,6 +278,15 @@ __global__ void __launch_bounds__(256) lattice_kernel(const LatticeParams p)
             }
 
             // L5: per-chain observables (integers until the final divide)
+            const bool alive = alive_i != 0u;
+            if (MIX) {   // lnW = ln 6 + sum_m count_m ln m, fixed order (the first step always has m = 6)
+                lnW = tab->ln_m[6];
+                lnW += (double)(hist & 255u) * tab->ln_m[2];
+                lnW += (double)((hist >> 8) & 255u) * tab->ln_m[3];
+                lnW += (double)((hist >> 16) & 255u) * tab->ln_m[4];
+                lnW += (double)(hist >> 24) * tab->ln_m[5];
+                if (!alive) lnW = -CUDART_INF;
+            }
             double ree2 = 0.0, rg2 = 0.0;
             if (alive) {
                 ree2 = (double)(hx * hx + hy * hy + hz * hz);
