@@ -322,21 +322,215 @@ __global__ void __launch_bounds__(256) lattice_kernel(const LatticeParams p)
     }
 }
 
-template <bool MIX, bool DIGEST, bool TRAJ>
-int launch_variant(const LatticeParams& p, cudaStream_t stream, int* grid_out)
+// =====================================================================================================
+// N <= 64: the byte-dot-product scan. Keys are plain integers with three 8-bit fields
+// biased by 128, so w = key_j - h is the integer dx + 256 dy + 65536 dz with |d| <= 126 < 2^7, a unique
+// balanced representation: monomer j sits on a neighbour site of h iff |w| is 1, 2^8 or 2^16, i.e. iff
+// exactly one byte of |w| is 1 and the rest are 0 (|w| < 2^24), i.e. iff dp4a.u8(|w|, |w|) == 1. The
+// scan XOR-accumulates w over those keys without a predicate: d = dp4a(|w|,|w|,-1) is 0 for a
+// neighbour and >= 1 otherwise, and w >> (32 d) keeps w or clears it (PTX shr clamps at 32). Every
+// neighbour site holds at most one monomer, so the XOR of {1, -1, 256, -256, 65536, -65536} over the
+// occupied subset decodes uniquely from bits 0,1,8,9,16,17 (table index, build_dp_tables).
+// Per key: IADD, IABS, IDP.4A, IMAD.SHL, SHF, 1/2 LOP3 -- 5.5 issue slots against 8 for the compare scan.
+// -----------------------------------------------------------------------------------------------------
+struct DpTables {
+    uint2    lut[64];   // index = (b0,b1,b8,b9,b16,b17) of the XOR. .x: bits 0-2 = m, bits 4+4i..6+4i = i-th free
+                        // direction; .y: histogram increment 1 << 8*(m-2) for m = 2..5
+    int32_t  delta[8];  // key delta per direction
+    double   ln_m[8];
+};
+
+__device__ __forceinline__ void build_dp_tables(DpTables* t)
+{
+    for (int idx = threadIdx.x; idx < 64; idx += blockDim.x) {
+        const int b0 = idx & 1, b1 = (idx >> 1) & 1, b8 = (idx >> 2) & 1, b9 = (idx >> 3) & 1, b16 = (idx >> 4) & 1, b17 = (idx >> 5) & 1;
+        // XOR patterns: +x 0x1, -x 0xFFFFFFFF, +y 0x100, -y 0xFFFFFF00, +z 0x10000, -z 0xFFFF0000
+        const int occ_d[6] = { b0 ^ b1, b1, b8 ^ b9, b9 ^ b1, b16 ^ b17, b17 ^ b9 };
+        uint32_t e = 0, m = 0;
+        for (int d = 0; d < 6; ++d)
+            if (!occ_d[d]) { e |= (uint32_t)d << (4 + 4 * m); ++m; }
+        t->lut[idx] = make_uint2(e | m, (m >= 2 && m <= 5) ? 1u << (8 * (m - 2)) : 0u);
+    }
+    if (threadIdx.x < 8) {
+        const int d = threadIdx.x;
+        t->delta[d] = d < 6 ? ((d & 1) ? -1 : 1) * (1 << (8 * (d >> 1))) : 0;
+        t->ln_m[d] = d == 0 ? -CUDART_INF : log((double)d);
+    }
+}
+
+#define ROSEN_DP_CHUNK(W)                                                                            \
+    "sub.s32 w0, " #W "0, %3; sub.s32 w1, " #W "1, %3; sub.s32 w2, " #W "2, %3; sub.s32 w3, " #W "3, %3;\n" \
+    "abs.s32 t0, w0; abs.s32 t1, w1; abs.s32 t2, w2; abs.s32 t3, w3;\n"                                \
+    "dp4a.u32.u32 t0, t0, t0, m1; dp4a.u32.u32 t1, t1, t1, m1; dp4a.u32.u32 t2, t2, t2, m1; dp4a.u32.u32 t3, t3, t3, m1;\n" \
+    "mul.lo.u32 t0, t0, 32; mul.lo.u32 t1, t1, 32; mul.lo.u32 t2, t2, 32; mul.lo.u32 t3, t3, 32;\n"    \
+    "shr.u32 w0, w0, t0; shr.u32 w1, w1, t1; shr.u32 w2, w2, t2; shr.u32 w3, w3, t3;\n"                \
+    "lop3.b32 A, A, w0, w1, 0x96; lop3.b32 A, A, w2, w3, 0x96;\n"
+
+// addr: shared byte address of the parity array, T >= 1 chunks of 4 keys, h: key of r_{s-1}. Returns the XOR.
+// Chunks are double-buffered; the load runs at most one chunk past the T-th (inside the thread's own region).
+__device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t h)
+{
+    uint32_t A;
+    asm volatile("{\n"
+        ".reg .pred q;\n"
+        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, A, m1, w0, w1, w2, w3, t0, t1, t2, t3;\n"
+        "mov.u32 ad, %1; mov.u32 cnt, %2; mov.u32 A, 0; mov.u32 m1, 0xFFFFFFFF;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
+        "DP_LOOP:\n"
+        "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
+        ROSEN_DP_CHUNK(a)
+        "setp.eq.u32 q, cnt, 1;\n"
+        "@q bra DP_DONE;\n"
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
+        ROSEN_DP_CHUNK(b)
+        "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
+        "setp.ne.u32 q, cnt, 0;\n"
+        "@q bra DP_LOOP;\n"
+        "DP_DONE:\n"
+        "mov.u32 %0, A;\n"
+        "}\n"
+        : "=r"(A)
+        : "r"(addr), "r"(T), "r"(h)
+        : "memory");
+    return A;
+}
+
+__device__ __forceinline__ uint2 lds64(uint32_t a) { uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t v) { asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" :: "r"(a), "r"(v), "r"(0u) : "memory"); }
+
+template <bool DIGEST, bool TRAJ>
+__global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    DpTables* tab = reinterpret_cast<DpTables*>(smem_raw);
+    Partial* scratch = reinterpret_cast<Partial*>(smem_raw + sizeof(DpTables));
+    uint32_t* chains = reinterpret_cast<uint32_t*>(smem_raw + sizeof(DpTables) + 8 * sizeof(Partial));
+
+    constexpr uint32_t kOrigin = 0x00808080u;
+    const int N = p.N;
+    const int half4 = half4_of(N), stride = stride_of(N);
+    uint32_t* ev = chains + (size_t)threadIdx.x * stride;   // monomers 0,2,4,...
+    uint32_t* od = ev + half4;                              // monomers 1,3,5,...
+    const uint32_t lut_addr = (uint32_t)__cvta_generic_to_shared(tab->lut);
+    const uint32_t delta_addr = (uint32_t)__cvta_generic_to_shared(tab->delta);
+    const uint32_t ev_addr = (uint32_t)__cvta_generic_to_shared(ev);
+    const uint32_t od_addr = ev_addr + (uint32_t)half4 * 4u;
+
+    build_dp_tables(tab);
+    __syncthreads();
+
+    const uint32_t per_thread = p.chunk / blockDim.x;
+
+    for (uint32_t vb = blockIdx.x; vb < p.n_vblocks; vb += gridDim.x) {
+        Partial acc = partial_zero();
+        for (uint32_t it = 0; it < per_thread; ++it) {
+            const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * blockDim.x + threadIdx.x;
+            if (idx >= p.n_chains) break;
+            const uint64_t chain = p.chain_offset + idx;
+            const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
+
+            // L0. No clearing pass: the first key of every 4-key chunk is stored as {key, 0, 0, 0}, so a scan
+            // never sees a key of the previous chain (0 is not a neighbour of any head: |0 - h| >= 0x414141).
+            uint32_t h = kOrigin;
+            sts128(ev_addr, h);
+            int sx = 0, sy = 0, sz = 0, s2 = 0;
+            uint32_t hist = 0, alive_i = 1u, steps = 0;
+            uint64_t dg = 0xCBF29CE484222325ull;
+            uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
+
+            for (int q = 0; 4 * q < N; ++q) {
+                uint32_t w[4];
+                philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.key0, p.key1, w);   // L1
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int s = 4 * q + k;
+                    if (s == 0 || s >= N) continue;
+
+                    // L2
+                    uint32_t A = 0;
+                    const uint32_t T = (uint32_t)(((s >> 1) + 3) >> 2);
+                    if (T != 0u) A = scan_dp((k & 1) ? od_addr : ev_addr, T, h);
+                    const uint32_t li = (((A & 0x00030303u) * 0x00010410u) >> 13) & 0x1F8u;   // 8 * (b0,b1,b8,b9,b16,b17)
+                    const uint2 le = lds64(lut_addr + li);
+                    const uint32_t m = le.x & 7u;
+
+                    // L3
+                    steps += alive_i;
+                    hist += le.y;
+                    if (TRAJ && mrow) mrow[s - 1] = alive_i ? (uint8_t)m : (uint8_t)0;
+
+                    // L4
+                    const uint32_t sel = __umulhi(w[k], m);
+                    const uint32_t d4 = (le.x >> (4u * sel + 2u)) & 0x1Cu;     // 4 * direction
+                    if (DIGEST) { if (alive_i) dg = digest_fold(dg, m, m ? (d4 >> 2) : 0xFFu); }
+                    alive_i &= min(m, 1u);
+                    h += lds32(delta_addr + d4);
+                    const uint32_t slot = ((k & 1) ? od_addr : ev_addr) + 4u * (uint32_t)(s >> 1);
+                    if (((s >> 1) & 3) == 0) sts128(slot, h); else sts32(slot, h);
+
+                    // L5: signed bytes of r_s; |r|^2 and the three coordinate sums as byte dot products
+                    const int sg = (int)(h ^ kOrigin);
+                    s2 = __dp4a(sg, sg, s2);
+                    sx = __dp4a(sg, 0x00000001, sx); sy = __dp4a(sg, 0x00000100, sy); sz = __dp4a(sg, 0x00010000, sz);
+                }
+            }
+
+            const bool alive = alive_i != 0u;
+            double lnW = tab->ln_m[6];
+            lnW += (double)(hist & 255u) * tab->ln_m[2];
+            lnW += (double)((hist >> 8) & 255u) * tab->ln_m[3];
+            lnW += (double)((hist >> 16) & 255u) * tab->ln_m[4];
+            lnW += (double)(hist >> 24) * tab->ln_m[5];
+            if (!alive) lnW = -CUDART_INF;
+            double ree2 = 0.0, rg2 = 0.0;
+            if (alive) {
+                const int sg = (int)(h ^ kOrigin);
+                ree2 = (double)__dp4a(sg, sg, 0);
+                const long long num = (long long)N * s2 - ((long long)sx * sx + (long long)sy * sy + (long long)sz * sz);
+                rg2 = (double)num / ((double)N * (double)N);
+            }
+            const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
+            acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
+            acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
+            if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
+
+            if (p.out.lnW) p.out.lnW[idx] = lnW;
+            if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
+            if (p.out.ree2) p.out.ree2[idx] = ree2;
+            if (p.out.rg2) p.out.rg2[idx] = rg2;
+            if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
+            if (TRAJ && p.out.conf) {
+                int32_t* c = reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3;
+                const int placed = alive ? N : (int)steps;
+                for (int i = 0; i < N; ++i) {
+                    const uint32_t v = ((i & 1) ? od : ev)[i >> 1];
+                    const bool ok = i < placed;
+                    c[3 * i + 0] = ok ? (int)(v & 255u) - 128 : 0;
+                    c[3 * i + 1] = ok ? (int)((v >> 8) & 255u) - 128 : 0;
+                    c[3 * i + 2] = ok ? (int)((v >> 16) & 255u) - 128 : 0;
+                }
+            }
+        }
+        block_reduce_store(acc, scratch, p.partials + vb);
+    }
+}
+
+template <typename Kern>
+int launch_kernel(Kern kern, size_t table_bytes, const LatticeParams& p, cudaStream_t stream, int* grid_out)
 {
     int dev = 0, n_sm = 0, smem_max = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const size_t fixed = sizeof(LatTables) + 8 * sizeof(Partial);
+    const size_t fixed = table_bytes + 8 * sizeof(Partial);
     const size_t per_thread = (size_t)stride_of(p.N) * 4;
     // threads per block depends on N only (never on the output variant): it fixes the reduction tree.
     int threads = 256;
     while (threads > 32 && fixed + per_thread * threads > (size_t)(72 * 1024)) threads >>= 1;
     const size_t smem = fixed + per_thread * threads;
     if (smem > (size_t)smem_max) return -2;
-    auto kern = lattice_kernel<MIX, DIGEST, TRAJ>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
@@ -348,6 +542,23 @@ int launch_variant(const LatticeParams& p, cudaStream_t stream, int* grid_out)
     if (cudaGetLastError() != cudaSuccess) return -3;
     *grid_out = grid;
     return 1;
+}
+
+template <bool MIX, bool DIGEST, bool TRAJ>
+int launch_variant(const LatticeParams& p, cudaStream_t stream, int* grid_out)
+{
+    return launch_kernel(lattice_kernel<MIX, DIGEST, TRAJ>, sizeof(LatTables), p, stream, grid_out);
+}
+
+int launch_dp(const LatticeParams& p, cudaStream_t stream, int* grid_out)
+{
+    const bool digest = p.out.digest != nullptr;
+    const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
+    const size_t tb = sizeof(DpTables);
+    if (traj) return digest ? launch_kernel(lattice_dp_kernel<true, true>, tb, p, stream, grid_out)
+                            : launch_kernel(lattice_dp_kernel<false, true>, tb, p, stream, grid_out);
+    return digest ? launch_kernel(lattice_dp_kernel<true, false>, tb, p, stream, grid_out)
+                  : launch_kernel(lattice_dp_kernel<false, false>, tb, p, stream, grid_out);
 }
 
 template <bool MIX>
@@ -365,6 +576,11 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
 {
     const bool digest = p.out.digest != nullptr;
     const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
+    if (p.N <= 64) {    // |dx|,|dy|,|dz| <= 126 fit signed bytes: byte-dot-product scan
+        *kernel_name = traj ? (digest ? "lattice_dp_kernel<digest,traj>" : "lattice_dp_kernel<traj>")
+                            : (digest ? "lattice_dp_kernel<digest>" : "lattice_dp_kernel");
+        return launch_dp(p, stream, grid_out);
+    }
     if (p.N <= 128) {   // keys < 2^24 are exact in fp32: mixed ISETP / fp32-product scan
         *kernel_name = traj ? (digest ? "lattice_kernel<mix,digest,traj>" : "lattice_kernel<mix,traj>")
                             : (digest ? "lattice_kernel<mix,digest>" : "lattice_kernel<mix>");
