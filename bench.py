@@ -52,11 +52,27 @@ def algorithmic_thread_instr(w: workloads.Workload) -> float:
         # 6 equality tests per site test + one Philox block (~70 instr) per 4 steps + ~20 per step for
         # count / weight / choose / place / observables
         return 6.0 * lattice_site_tests(w.N) + 70.0 * ((w.N + 3) // 4) + 20.0 * (w.N - 1)
-    # real space, full pair scan of Alg. 2: k (N-1)(N-2)/2 pair tests x 7 instr + k/2 Philox blocks and k
-    # direction evaluations (~45 instr) per step + ~30 per step
+    # real space after the exact candidate reduction (DESIGN.md 5.2 / 6): (N-1)(N-2)/2 prefilter tests and
+    # k * c pair tests per step with c = 3.2 candidates on average, 7 instr each, + k/2 Philox
+    # blocks (35 per trial) and k direction evaluations (45) per step + ~30 per step
     k, N = w.k_trials, w.N
-    pairs = k * (N - 1) * (N - 2) / 2.0
-    return 7.0 * pairs + (N - 1) * (35.0 * k + 45.0 * k + 30.0)
+    return 7.0 * (N - 1) * (N - 2) / 2.0 + (N - 1) * (7.0 * 3.2 * k + 35.0 * k + 45.0 * k + 30.0)
+
+
+def profile_traffic(w: workloads.Workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu summary of
+    this workload (profiles/), per launch; None if no capture is committed."""
+    name = {"lattice_N64_2p24": "r01c_lattice_cfg2_dp.md", "realspace_N64_k16_2p22": "r01b_realspace_cfg3.md"}.get(w.name)
+    path = os.path.join(ROOT, "profiles", name) if name else None
+    if not path or not os.path.exists(path):
+        return None
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total = 0.0
+    for line in open(path):
+        cells = [c.strip() for c in line.split("|")]
+        if len(cells) >= 4 and cells[1] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            total += float(cells[3]) * mult.get(cells[2], 1.0)
+    return total
 
 
 def load_measured_peaks():
@@ -262,6 +278,24 @@ def run_product(args, w, rank, world, local_rank):
     kms = timed(lambda: enqueue(None), max(3, min(steps, 10)))
     kernel_ms = sum(kms) / len(kms)
 
+    # ---- dump path (config 5): store phase D1 in situ = time(generation + dump) - time(generation only), same
+    # launch geometry and lane mapping; bytes stored / that difference = achieved HBM write GB/s of the store phase
+    dump_info = None
+    if w.dump and w.kind == "realspace":
+        def gen_only():
+            R.rosen_realspace_generate_async(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, offset,
+                                             outputs=None, summary_device=None, stream=stream)
+        timed(gen_only, 1)
+        t_gen = min(timed(gen_only, 3))
+        t_all = min(kms)
+        nbytes = w.n_chains * (12 * w.N + 8)
+        diff = t_all - t_gen
+        resolved = diff > 0.01 * t_all          # below 1 % of the call the difference is timing noise
+        dump_info = {"bytes_per_step": nbytes, "with_dump_ms": t_all, "generation_only_ms": t_gen, "store_phase_ms": diff,
+                     "achieved_GBps": nbytes / (diff * 1e-3) / 1e9 if resolved else None,
+                     "whole_call_GBps": nbytes / (t_all * 1e-3) / 1e9,
+                     "note": None if resolved else "store phase not resolvable: hidden under generation (compute-bound call)"}
+
     # ---- end-to-end leg: synchronous C-ABI call, host buffers ------------------------------------
     for _ in range(2):
         sync_call()
@@ -296,7 +330,7 @@ def run_product(args, w, rank, world, local_rank):
     alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
     achieved = alg_winst / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
-                "frac": achieved / peak_winst, "traffic": None, "kernel": kernel_name, "kernel_ms": kernel_ms,
+                "frac": achieved / peak_winst, "traffic": profile_traffic(w), "kernel": kernel_name, "kernel_ms": kernel_ms,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
                 "algorithmic_thread_instr_per_chain": algorithmic_thread_instr(w)}
     if clocks.get("sm_mhz"):
@@ -320,6 +354,10 @@ def run_product(args, w, rank, world, local_rank):
                         + (" + host conf/lnW" if w.dump else "")},
         "gpu_launches": launches_per_step * steps,
     }
+    if dump_info is not None:
+        dump_info["peak_GBps"] = float(peaks.get("hbm_gbs", 6650.0))
+        dump_info["frac"] = dump_info["achieved_GBps"] / dump_info["peak_GBps"] if dump_info["achieved_GBps"] else None
+        out["dump_path"] = dump_info
     if world == 1 and not args.no_cpu_baseline:
         m, dt, _ = time_oracle(w, args.cpu_seconds)
         out["cpu_baseline"] = {"value": m / dt, "unit": "chains/s", "cores": 1, "kind": "oracle",

@@ -58,12 +58,12 @@ __device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t
 // shared memory carve-up (bytes) -----------------------------------------------------------------
 //   double   ln_tab[256]            ln m, ln_tab[0] = -inf
 //   Partial  scratch[32]
-//   per group: float x[Np], y[Np], z[Np]; uint16 cand[Np]; uint8 mseq[Np]   (Np = N rounded up to 4)
+//   per group: float4 r[Np] (x, y, z, unused); uint16 cand[Np] (byte offsets into r); uint8 mseq[Np]   (Np = N rounded up to 4)
 __host__ __device__ inline int n_pad(int N) { return (N + 3) & ~3; }
-__host__ __device__ inline size_t group_bytes(int N) { return (size_t)n_pad(N) * (12 + 2 + 1) + 4; }
+__host__ __device__ inline size_t group_bytes(int N) { return (size_t)n_pad(N) * (16 + 2 + 1) + 4; }
 
 template <int G, int P, bool DIGEST, bool TRAJ>
-__global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
+__global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const RealParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* ln_tab = reinterpret_cast<double*>(smem_raw);
@@ -78,10 +78,8 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
     const uint32_t below = (1u << gl) - 1u;
     const int group_in_block = threadIdx.x / G;
     const size_t gsz = (group_bytes(N) + 15) & ~(size_t)15;
-    float* X = reinterpret_cast<float*>(gbase_ptr + gsz * group_in_block);
-    float* Y = X + Np;
-    float* Z = Y + Np;
-    uint16_t* cand = reinterpret_cast<uint16_t*>(Z + Np);
+    float4* R4 = reinterpret_cast<float4*>(gbase_ptr + gsz * group_in_block);   // one LDS.128 per monomer
+    uint16_t* cand = reinterpret_cast<uint16_t*>(R4 + Np);
     uint8_t* mbuf = reinterpret_cast<uint8_t*>(cand + Np);
 
     for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
@@ -101,16 +99,21 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
 
         // R0
         float hx = 0.f, hy = 0.f, hz = 0.f;
-        if (gl == 0) { X[0] = 0.f; Y[0] = 0.f; Z[0] = 0.f; }
+        if (gl == 0) R4[0] = make_float4(0.f, 0.f, 0.f, 0.f);
         double lnW = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0, S2 = 0.0;
         bool alive = true;
         uint32_t steps = 0;
         uint64_t dg = 0xCBF29CE484222325ull;
         uint32_t selw[4] = {0, 0, 0, 0};
+        uint32_t usel = 0;
         __syncwarp();
 
         for (int s = 1; s < N; ++s) {
             if ((s & 3) == 0 || s == 1) philox4x32_10(c_lo, c_hi, (uint32_t)(s >> 2), 0u, p.key0, p.key1, selw);
+            {   // word s & 3 without a dynamically indexed (local-memory) array
+                const uint32_t lo = (s & 1) ? selw[1] : selw[0], hi = (s & 1) ? selw[3] : selw[2];
+                usel = (s & 2) ? hi : lo;
+            }
 
             // ---- candidates: monomers j <= s-2 within the conservative radius of r_{s-1}
             int ncand = 0;
@@ -118,11 +121,12 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
                 const int j = j0 + gl;
                 bool in = false;
                 if (j < s - 1) {
-                    const float dx = X[j] - hx, dy = Y[j] - hy, dz = Z[j] - hz;
+                    const float4 rj = R4[j];
+                    const float dx = rj.x - hx, dy = rj.y - hy, dz = rj.z - hz;
                     in = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < p.prefilter2;
                 }
                 const uint32_t bits = (__ballot_sync(0xffffffffu, in) >> gshift) & gmask;
-                if (in) cand[ncand + __popc(bits & below)] = (uint16_t)j;
+                if (in) cand[ncand + __popc(bits & below)] = (uint16_t)(j * 16);
                 ncand += __popc(bits);
             }
             __syncwarp();
@@ -146,8 +150,8 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
                 }
             }
             for (int c = 0; c < ncand; ++c) {
-                const int j = cand[c];
-                const float xj = X[j], yj = Y[j], zj = Z[j];
+                const float4 rj = *reinterpret_cast<const float4*>(reinterpret_cast<const unsigned char*>(R4) + cand[c]);
+                const float xj = rj.x, yj = rj.y, zj = rj.z;
 #pragma unroll
                 for (int pp = 0; pp < P; ++pp)
 #pragma unroll
@@ -175,7 +179,7 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
             if (TRAJ) { if (gl == 0) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
 
             // ---- R4: the sel-th free trial
-            const uint32_t sel = __umulhi(selw[s & 3], m);
+            const uint32_t sel = __umulhi(usel, m);
             uint32_t base = 0;
             bool hit = false;
             float px = hx, py = hy, pz = hz;
@@ -195,7 +199,7 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
             if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? tsel : 0xFFu); }
             alive = alive && (m != 0u);
             if (m != 0u) { hx = px; hy = py; hz = pz; }
-            if (gl == 0) { X[s] = hx; Y[s] = hy; Z[s] = hz; }
+            if (gl == 0) R4[s] = make_float4(hx, hy, hz, 0.f);
 
             // ---- R5 running sums (fp64)
             Sx += (double)hx; Sy += (double)hy; Sz += (double)hz;
@@ -228,7 +232,7 @@ __global__ void __launch_bounds__(256) realspace_kernel(const RealParams p)
                 float* c = reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3;
                 for (int e = gl; e < 3 * N; e += G) {
                     const int i = e / 3, a = e - 3 * i;
-                    const float v = a == 0 ? X[i] : (a == 1 ? Y[i] : Z[i]);
+                    const float v = reinterpret_cast<const float*>(R4)[4 * i + a];
                     c[e] = i < placed ? v : 0.0f;
                 }
             }
