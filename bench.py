@@ -367,6 +367,46 @@ def run_product(args, w, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE config 4: lattice length sweep N in {8..256}, 2^24 chains each, seed 11: attrition(N), nu from
+    <Ree2> ~ (N-1)^(2 nu) (least squares on logs, reading A14), throughput per N. One JSON line."""
+    import math
+
+    import torch
+    import paper_1704_04381_b200 as R
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    R.load_library()
+    stream = torch.cuda.Stream()
+    summary_dev = torch.zeros(R.SUMMARY_BYTES, dtype=torch.uint8, device="cuda")
+    rows = []
+    for w in workloads.CONFIG_4:
+        def call():
+            R.rosen_lattice_generate_async(w.N, w.n_chains, w.seed, 0, outputs=None, summary_device=summary_dev, stream=stream)
+        ms = []
+        with torch.cuda.stream(stream):
+            for i in range(2 + max(args.steps, 1)):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); call(); b.record(stream)
+                ms.append((a, b))
+        stream.synchronize()
+        t = [a.elapsed_time(b) for a, b in ms][2:]
+        sm = R.summary_from_device(summary_dev)
+        best = min(t)
+        rows.append({"N": w.N, "ms": best, "chains_per_s": w.n_chains / (best * 1e-3),
+                     "monomer_steps_per_s": sm["n_steps_attempted"] / (best * 1e-3), "attrition": sm["attrition"],
+                     "mean_ree2": sm["mean_ree2"], "mean_rg2": sm["mean_rg2"], "ln_mean_W": sm["ln_mean_W"],
+                     "ess_fraction": sm["sum_w"] ** 2 / sm["sum_w2"] / sm["n_chains"], "kernel": R.rosen_last_kernel_name()})
+    xs = [math.log(r["N"] - 1) for r in rows]; ys = [math.log(r["mean_ree2"]) for r in rows]
+    n = len(xs); mx, my = sum(xs) / n, sum(ys) / n
+    slope = sum((x - mx) * (y - my) for x, y in zip(xs, ys)) / sum((x - mx) ** 2 for x in xs)
+    # mu from ln<W>_N - ln<W>_{N/2} over the last octave (Eq. 5-6, PAPER.md:356-362), crude two-point estimate
+    mu = math.exp((rows[-1]["ln_mean_W"] - rows[-2]["ln_mean_W"]) / (rows[-1]["N"] - rows[-2]["N"]))
+    print(json.dumps({"metric": "lattice length sweep (BASELINE config 4)", "seed": workloads.CONFIG_4[0].seed,
+                      "n_chains": workloads.CONFIG_4[0].n_chains, "nu_fit": slope / 2.0, "mu_two_point": mu,
+                      "sweep": rows, "data": "synthetic"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -376,11 +416,16 @@ def main():
     ap.add_argument("--impl", default="product", choices=("product", "reference"))
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="run BASELINE config 4 (length sweep) instead")
     args = ap.parse_args()
     w = workloads.CONFIGS[args.workload]
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+        return
     if args.impl == "reference":
         run_reference(args, w, rank)
     else:

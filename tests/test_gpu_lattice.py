@@ -161,3 +161,28 @@ def test_config2_full_size_sampled(R):
     assert int(d64.sum()) & (2 ** 64 - 1) == s["digest_sum"]     # int64 wrap-around sum == uint64 sum mod 2^64
     # physics sanity (loose): attrition ~3.6e-3, nu-consistent <Ree2> ~ 152
     assert 2e-3 < s["attrition"] < 6e-3 and 140 < s["mean_ree2"] < 165
+
+
+def test_config4_sweep_reduced(R):
+    """BASELINE config 4 (length sweep, seed 11) at 2^18 chains per N: kernel variant per N, sampled per-chain
+    parity against the oracle, attrition grows with N, nu from <Ree2> ~ (N-1)^(2 nu) in the paper's band
+    (PAPER.md:350 0.601 text / :374 0.588 table; [0.58, 0.62])."""
+    n = 1 << 18
+    xs, ys, att = [], [], []
+    for N in workloads.CONFIG_4_N:
+        s, t = R.rosen_lattice_generate(N, n, 11, outputs=("digest", "lnW", "alive", "ree2"))
+        name = R.rosen_last_kernel_name()
+        assert name.startswith("lattice_dp_kernel") if N <= 64 else name.startswith("lattice_kernel<mix") if N <= 128 \
+            else name.startswith("lattice_kernel<int")
+        pre = 384
+        o = oracle.lattice_generate(N, pre, 11, outputs=("digest", "lnW", "alive", "ree2"))
+        assert np.array_equal(t["digest"][:pre].cpu().numpy().view(np.uint64), o.digest)
+        assert np.array_equal(t["alive"][:pre].cpu().numpy(), o.alive)
+        assert np.array_equal(t["ree2"][:pre].cpu().numpy(), o.ree2)
+        tail = oracle.lattice_generate(N, 2, 11, chain_offset=n - 2, outputs=("digest",))
+        assert np.array_equal(t["digest"][n - 2:].cpu().numpy().view(np.uint64), tail.digest)
+        xs.append(math.log(N - 1)); ys.append(math.log(s["mean_ree2"])); att.append(s["attrition"])
+    assert att[0] == 0.0 and all(a <= b for a, b in zip(att, att[1:])) and 0.02 < att[-1] < 0.06
+    mx, my = sum(xs) / len(xs), sum(ys) / len(ys)
+    nu = 0.5 * sum((x - mx) * (y - my) for x, y in zip(xs, ys)) / sum((x - mx) ** 2 for x in xs)
+    assert 0.57 < nu < 0.63, nu
