@@ -172,8 +172,7 @@ def test_config4_sweep_reduced(R):
     for N in workloads.CONFIG_4_N:
         s, t = R.rosen_lattice_generate(N, n, 11, outputs=("digest", "lnW", "alive", "ree2"))
         name = R.rosen_last_kernel_name()
-        assert name.startswith("lattice_dp_kernel") if N <= 64 else name.startswith("lattice_kernel<mix") if N <= 128 \
-            else name.startswith("lattice_kernel<int")
+        assert name.startswith("lattice_dp_kernel<wide") if N > 64 else name.startswith("lattice_dp_kernel") and "wide" not in name
         pre = 384
         o = oracle.lattice_generate(N, pre, 11, outputs=("digest", "lnW", "alive", "ree2"))
         assert np.array_equal(t["digest"][:pre].cpu().numpy().view(np.uint64), o.digest)
