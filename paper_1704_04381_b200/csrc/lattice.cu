@@ -70,9 +70,10 @@ __device__ __forceinline__ void build_dp_tables(DpTables* t)
     "sub.s32 w0, " #W "0, %3; sub.s32 w1, " #W "1, %3; sub.s32 w2, " #W "2, %3; sub.s32 w3, " #W "3, %3;\n" \
     "abs.s32 t0, w0; abs.s32 t1, w1; abs.s32 t2, w2; abs.s32 t3, w3;\n"                                \
     "dp4a.u32.u32 t0, t0, t0, m1; dp4a.u32.u32 t1, t1, t1, m1; dp4a.u32.u32 t2, t2, t2, m1; dp4a.u32.u32 t3, t3, t3, m1;\n" \
-    "mul.lo.u32 t0, t0, 32; mul.lo.u32 t1, t1, 32; mul.lo.u32 t2, t2, 32; mul.lo.u32 t3, t3, 32;\n"    \
-    "shr.u32 w0, w0, t0; shr.u32 w1, w1, t1; shr.u32 w2, w2, t2; shr.u32 w3, w3, t3;\n"                \
-    "lop3.b32 A, A, w0, w1, 0x96; lop3.b32 A, A, w2, w3, 0x96;\n"
+    "mul.lo.u32 t0, t0, 32; mul.lo.u32 t2, t2, 32;\n"                                                  \
+    "shr.u32 w0, w0, t0; shr.u32 w2, w2, t2;\n"                                                        \
+    "setp.eq.u32 p1, t1, 0; setp.eq.u32 p3, t3, 0;\n"                                                  \
+    "lop3.b32 A, A, w0, w2, 0x96; @p1 xor.b32 A, A, w1; @p3 xor.b32 A, A, w3;\n"
 
 // addr: shared byte address of the parity array, T >= 1 chunks of 4 keys, h: key of r_{s-1}. Returns the XOR.
 // Chunks are double-buffered; the load runs at most one chunk past the T-th (inside the thread's own region).
@@ -80,15 +81,22 @@ __device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t 
 {
     uint32_t A;
     asm volatile("{\n"
-        ".reg .pred q;\n"
-        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, A, m1, w0, w1, w2, w3, t0, t1, t2, t3;\n"
+        ".reg .pred q, p1, p3;\n"
+        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, od, cnt, A, m1, w0, w1, w2, w3, t0, t1, t2, t3;\n"
         "mov.u32 ad, %1; mov.u32 cnt, %2; mov.u32 A, 0; mov.u32 m1, 0xFFFFFFFF;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
+        "and.b32 od, cnt, 1;\n"
+        "setp.eq.u32 q, od, 0;\n"
+        "@q bra DP_EVEN;\n"                      // odd T: peel one chunk, then whole pairs without a mid-loop exit
+        ROSEN_DP_CHUNK(a)
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+16];\n"
+        "add.u32 ad, ad, 16; sub.u32 cnt, cnt, 1;\n"
+        "DP_EVEN:\n"
+        "setp.eq.u32 q, cnt, 0;\n"
+        "@q bra DP_DONE;\n"
         "DP_LOOP:\n"
         "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
         ROSEN_DP_CHUNK(a)
-        "setp.eq.u32 q, cnt, 1;\n"
-        "@q bra DP_DONE;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
         ROSEN_DP_CHUNK(b)
         "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
