@@ -297,7 +297,8 @@ int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kern
     if (blocks <= 1)  { *kernel_name = "realspace_kernel<G=1,P=1>";  return launch_gp<1, 1>(p, stream, grid_out); }
     if (blocks <= 2)  { *kernel_name = "realspace_kernel<G=2,P=1>";  return launch_gp<2, 1>(p, stream, grid_out); }
     if (blocks <= 4)  { *kernel_name = "realspace_kernel<G=4,P=1>";  return launch_gp<4, 1>(p, stream, grid_out); }
-    if (blocks <= 8)  { *kernel_name = "realspace_kernel<G=8,P=1>";  return launch_gp<8, 1>(p, stream, grid_out); }
+    // 5..8 blocks: 4 lanes x 2 blocks per lane measured 8 % faster than 8 x 1 (config 3: 41.5 -> 38.1 ms)
+    if (blocks <= 8)  { *kernel_name = "realspace_kernel<G=4,P=2>";  return launch_gp<4, 2>(p, stream, grid_out); }
     if (blocks <= 16) { *kernel_name = "realspace_kernel<G=16,P=1>"; return launch_gp<16, 1>(p, stream, grid_out); }
     if (blocks <= 32) { *kernel_name = "realspace_kernel<G=32,P=1>"; return launch_gp<32, 1>(p, stream, grid_out); }
     if (blocks <= 64) { *kernel_name = "realspace_kernel<G=32,P=2>"; return launch_gp<32, 2>(p, stream, grid_out); }
