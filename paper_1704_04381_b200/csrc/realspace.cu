@@ -293,7 +293,17 @@ int launch_gp(const RealParams& p, cudaStream_t stream, int* grid_out)
 
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out)
 {
-    const int blocks = (p.k + 1) / 2;   // Philox blocks (trial pairs) per step
+    int blocks = (p.k + 1) / 2;   // Philox blocks (trial pairs) per step
+    // Long chains: a warp holds 32/G chains of group_bytes(N) each; widen the group (idle lanes own trials >= k)
+    // until one warp's chains fit 24 KB, so that a block of >= 4 warps fits shared memory up to N = 1024.
+    {
+        const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
+        int g_mem = 1;
+        while (g_mem < 32 && (32 / g_mem) * gsz > (size_t)(24 * 1024)) g_mem *= 2;
+        if (g_mem > 4 && blocks < g_mem) blocks = g_mem;      // selects <G = g_mem, P = 1> below (g_mem = 8 -> G = 16)
+        else if (g_mem > 1 && blocks < g_mem) blocks = g_mem; // 2 or 4
+        if (g_mem == 8 && blocks <= 8) blocks = 9;            // no <8,1> variant: take <16,1>
+    }
     if (blocks <= 1)  { *kernel_name = "realspace_kernel<G=1,P=1>";  return launch_gp<1, 1>(p, stream, grid_out); }
     if (blocks <= 2)  { *kernel_name = "realspace_kernel<G=2,P=1>";  return launch_gp<2, 1>(p, stream, grid_out); }
     if (blocks <= 4)  { *kernel_name = "realspace_kernel<G=4,P=1>";  return launch_gp<4, 1>(p, stream, grid_out); }

@@ -72,6 +72,7 @@ def test_config5_prefix(R):
     (40, 300, 32, 2.0, 1.7, 9, 0), (31, 300, 33, 1.0, 1.0, 10, 0), (25, 300, 64, 1.0, 1.0, 10, 0),
     (25, 200, 65, 1.0, 0.8, 11, 0), (20, 150, 128, 1.0, 1.0, 11, 0), (18, 100, 129, 1.0, 1.0, 12, 0),
     (12, 100, 255, 1.0, 1.0, 12, 0), (130, 64, 16, 1.0, 1.0, 13, 0), (64, 2000, 16, 1.0, 1.9, 14, 0),
+    (1024, 6, 4, 1.0, 0.6, 15, 0), (1024, 3, 2, 0.5, 0.0, 15, 2),        # ROSEN_REALSPACE_MAX_N
 ])
 def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
     check(R, N, n, k, b, sigma, seed, offset)
