@@ -397,13 +397,11 @@ def run_sweep(args):
                      "monomer_steps_per_s": sm["n_steps_attempted"] / (best * 1e-3), "attrition": sm["attrition"],
                      "mean_ree2": sm["mean_ree2"], "mean_rg2": sm["mean_rg2"], "ln_mean_W": sm["ln_mean_W"],
                      "ess_fraction": sm["sum_w"] ** 2 / sm["sum_w2"] / sm["n_chains"], "kernel": R.rosen_last_kernel_name()})
-    xs = [math.log(r["N"] - 1) for r in rows]; ys = [math.log(r["mean_ree2"]) for r in rows]
-    n = len(xs); mx, my = sum(xs) / n, sum(ys) / n
-    slope = sum((x - mx) * (y - my) for x, y in zip(xs, ys)) / sum((x - mx) ** 2 for x in xs)
-    # mu from ln<W>_N - ln<W>_{N/2} over the last octave (Eq. 5-6), crude two-point estimate
-    mu = math.exp((rows[-1]["ln_mean_W"] - rows[-2]["ln_mean_W"]) / (rows[-1]["N"] - rows[-2]["N"]))
+    fit = R.rosen_fit_exponents([r["N"] for r in rows], [r["mean_ree2"] for r in rows], [r["ln_mean_W"] for r in rows],
+                                use_steps=True)                    # Eq. 4-7, x = N - 1 (reading A14)
+    slope, mu = 2.0 * fit["nu"], fit["mu"]
     print(json.dumps({"metric": "lattice length sweep (BASELINE config 4)", "seed": workloads.CONFIG_4[0].seed,
-                      "n_chains": workloads.CONFIG_4[0].n_chains, "nu_fit": slope / 2.0, "mu_two_point": mu,
+                      "n_chains": workloads.CONFIG_4[0].n_chains, "nu_fit": slope / 2.0, "mu_fit": mu, "gamma_fit": fit["gamma"], "fit": fit,
                       "sweep": rows, "data": "synthetic"}))
 
 

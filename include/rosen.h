@@ -140,6 +140,25 @@ ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trial
  */
 ROSEN_API int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged);
 
+/*
+ * Scaling analysis of a length sweep (sec. 4.1: Eq. 4 <R_N^2> = a N^(2 nu); Eq. 5-7
+ * ln Z_N ~ N ln mu + (gamma - 1) ln N with Z_N = <W_N>, Eq. 6). Ordinary least squares over `count` lengths:
+ *   ln mean_ree2[i] = ln a + 2 nu ln x_i                       (count >= 2)
+ *   ln_mean_W[i]    = c + x_i ln mu + (gamma - 1) ln x_i       (count >= 3; skipped, fields NaN, if count == 2)
+ * with x_i = N[i] - 1 (number of steps; reading A14 of DESIGN.md 4) if use_steps != 0, else x_i = N[i].
+ * Pure host function over the summaries of rosen_lattice_generate / rosen_realspace_generate calls
+ * (ln_mean_W of real space must have (N-1) ln k subtracted by the caller if mu per trial is wanted).
+ * Returns ROSEN_EINVAL on count < 2, N[i] < 2, non-positive mean_ree2, non-finite input or a singular system.
+ */
+typedef struct rosen_fit {
+    double nu, ln_a;              /* Eq. 4 */
+    double mu, gamma, c;          /* Eq. 5-7 */
+    double rms_ree2, rms_lnZ;     /* root-mean-square residuals of the two fits (log scale) */
+} rosen_fit;
+
+ROSEN_API int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double* ln_mean_W,
+                                  int32_t count, int32_t use_steps, rosen_fit* fit);
+
 /* Bytes of device scratch the library keeps per device for block partials (informational). */
 ROSEN_API size_t rosen_workspace_bytes(void);
 

@@ -151,3 +151,19 @@ def saw_enumerate(n: int, fix_first: bool = False) -> dict:
     mult = 6 if fix_first else 1
     h = {tuple(int(i) for i in idx): int(hist[tuple(idx)]) * mult for idx in np.argwhere(hist)}
     return {"count": cnt.value * mult, "sum_ree2": s1.value * mult, "sum_n2rg2": s2.value * mult, "hist": h}
+
+
+def fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> dict:
+    """Scaling analysis of a length sweep, PAPER.md:342-367 (sec. 4.1): Eq. 4 <R_N^2> = a N^(2 nu) and
+    Eq. 7 ln Z_N = c + N ln mu + (gamma - 1) ln N with Z_N = <W_N> (Eq. 6), each as the plain linear
+    least-squares problem it states, solved by numpy.linalg.lstsq. x = N - 1 when use_steps (reading A14)."""
+    x = np.asarray(N, dtype=np.float64) - (1.0 if use_steps else 0.0)
+    lx = np.log(x)
+    A1 = np.stack([np.ones_like(lx), lx], axis=1)
+    (ln_a, slope), *_ = np.linalg.lstsq(A1, np.log(np.asarray(mean_ree2, dtype=np.float64)), rcond=None)
+    out = {"nu": 0.5 * slope, "ln_a": ln_a, "mu": float("nan"), "gamma": float("nan"), "c": float("nan")}
+    if len(x) >= 3:
+        A2 = np.stack([np.ones_like(lx), x, lx], axis=1)
+        (c, ln_mu, gm1), *_ = np.linalg.lstsq(A2, np.asarray(ln_mean_W, dtype=np.float64), rcond=None)
+        out.update(mu=float(np.exp(ln_mu)), gamma=float(gm1 + 1.0), c=float(c))
+    return out

@@ -246,6 +246,24 @@ def rosen_summary_merge(parts) -> Dict[str, float]:
     return out.as_dict()
 
 
+class rosen_fit(C.Structure):
+    _fields_ = [("nu", C.c_double), ("ln_a", C.c_double), ("mu", C.c_double), ("gamma", C.c_double), ("c", C.c_double),
+                ("rms_ree2", C.c_double), ("rms_lnZ", C.c_double)]
+
+
+def rosen_fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> Dict[str, float]:
+    """rosen_fit_exponents: nu (Eq. 4) and mu, gamma (Eq. 5-7) by least squares over a length sweep."""
+    L = load_library()
+    n = len(N)
+    L.rosen_fit_exponents.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int32,
+                                      C.c_int32, C.POINTER(rosen_fit)]
+    L.rosen_fit_exponents.restype = C.c_int
+    out = rosen_fit()
+    _check(L.rosen_fit_exponents((C.c_int32 * n)(*[int(v) for v in N]), (C.c_double * n)(*[float(v) for v in mean_ree2]),
+                                 (C.c_double * n)(*[float(v) for v in ln_mean_W]), n, 1 if use_steps else 0, C.byref(out)))
+    return {name: getattr(out, name) for name, _ in out._fields_}
+
+
 def rosen_workspace_bytes() -> int:
     return int(load_library().rosen_workspace_bytes())
 

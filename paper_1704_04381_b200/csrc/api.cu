@@ -280,6 +280,49 @@ int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary
     return ROSEN_OK;
 }
 
+int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double* ln_mean_W,
+                        int32_t count, int32_t use_steps, rosen_fit* fit)
+{
+    if (!N || !mean_ree2 || !ln_mean_W || !fit || count < 2) return ROSEN_EINVAL;
+    const double nan = std::nan("");
+    // normal equations of y = p0 + p1 x + p2 lx  (Eq. 7) and of r = q0 + q1 lx (Eq. 4), centred for conditioning
+    double mx = 0, ml = 0, my = 0, mr = 0;
+    for (int32_t i = 0; i < count; ++i) {
+        if (N[i] < 2 || !(mean_ree2[i] > 0.0) || !std::isfinite(mean_ree2[i]) || !std::isfinite(ln_mean_W[i])) return ROSEN_EINVAL;
+        const double x = (double)(N[i] - (use_steps ? 1 : 0));
+        mx += x; ml += std::log(x); my += ln_mean_W[i]; mr += std::log(mean_ree2[i]);
+    }
+    mx /= count; ml /= count; my /= count; mr /= count;
+    double sxx = 0, sxl = 0, sll = 0, sxy = 0, sly = 0, slr = 0;
+    for (int32_t i = 0; i < count; ++i) {
+        const double x = (double)(N[i] - (use_steps ? 1 : 0));
+        const double dx = x - mx, dl = std::log(x) - ml, dy = ln_mean_W[i] - my, dr = std::log(mean_ree2[i]) - mr;
+        sxx += dx * dx; sxl += dx * dl; sll += dl * dl; sxy += dx * dy; sly += dl * dy; slr += dl * dr;
+    }
+    if (!(sll > 0.0)) return ROSEN_EINVAL;
+    rosen_fit f;
+    const double slope = slr / sll;
+    f.nu = 0.5 * slope; f.ln_a = mr - slope * ml;
+    f.mu = f.gamma = f.c = f.rms_lnZ = nan;
+    double p1 = 0, p2 = 0;
+    if (count >= 3) {
+        const double det = sxx * sll - sxl * sxl;
+        if (!(std::fabs(det) > 1e-14 * sxx * sll)) return ROSEN_EINVAL;
+        p1 = (sxy * sll - sly * sxl) / det; p2 = (sly * sxx - sxy * sxl) / det;
+        f.mu = std::exp(p1); f.gamma = p2 + 1.0; f.c = my - p1 * mx - p2 * ml;
+    }
+    double e1 = 0, e2 = 0;
+    for (int32_t i = 0; i < count; ++i) {
+        const double x = (double)(N[i] - (use_steps ? 1 : 0)), lx = std::log(x);
+        const double r1 = std::log(mean_ree2[i]) - (f.ln_a + slope * lx); e1 += r1 * r1;
+        if (count >= 3) { const double r2 = ln_mean_W[i] - (f.c + p1 * x + p2 * lx); e2 += r2 * r2; }
+    }
+    f.rms_ree2 = std::sqrt(e1 / count);
+    if (count >= 3) f.rms_lnZ = std::sqrt(e2 / count);
+    *fit = f;
+    return ROSEN_OK;
+}
+
 size_t rosen_workspace_bytes(void) { return sizeof(Partial) * rosen::kMaxPartials + sizeof(rosen_summary); }
 int32_t rosen_last_launch_count(void) { return g_launches; }
 const char* rosen_last_kernel_name(void) { return g_kernel; }
