@@ -116,18 +116,22 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
             }
 
             // ---- candidates: monomers j <= s-2 within the conservative radius of r_{s-1}
+            // (two monomers per lane and iteration: independent loads and distance chains hide each other's latency;
+            // the order of the list is irrelevant, overlap is an OR over candidates)
             int ncand = 0;
-            for (int j0 = 0; j0 < s - 1; j0 += G) {
-                const int j = j0 + gl;
-                bool in = false;
-                if (j < s - 1) {
-                    const float4 rj = R4[j];
-                    const float dx = rj.x - hx, dy = rj.y - hy, dz = rj.z - hz;
-                    in = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < p.prefilter2;
-                }
-                const uint32_t bits = (__ballot_sync(0xffffffffu, in) >> gshift) & gmask;
-                if (in) cand[ncand + __popc(bits & below)] = (uint16_t)(j * 16);
-                ncand += __popc(bits);
+            for (int j0 = 0; j0 < s - 1; j0 += 2 * G) {
+                const int ja = j0 + gl, jb = ja + G;
+                const float4 ra = R4[min(ja, s - 2)], rb = R4[min(jb, s - 2)];
+                const float ax = ra.x - hx, ay = ra.y - hy, az = ra.z - hz;
+                const float bx = rb.x - hx, by = rb.y - hy, bz = rb.z - hz;
+                const bool ina = ja < s - 1 && fmaf(az, az, fmaf(ay, ay, ax * ax)) < p.prefilter2;
+                const bool inb = jb < s - 1 && fmaf(bz, bz, fmaf(by, by, bx * bx)) < p.prefilter2;
+                const uint32_t bita = (__ballot_sync(0xffffffffu, ina) >> gshift) & gmask;
+                const uint32_t bitb = (__ballot_sync(0xffffffffu, inb) >> gshift) & gmask;
+                const int na = __popc(bita);
+                if (ina) cand[ncand + __popc(bita & below)] = (uint16_t)(ja * 16);
+                if (inb) cand[ncand + na + __popc(bitb & below)] = (uint16_t)(jb * 16);
+                ncand += na + __popc(bitb);
             }
             __syncwarp();
 
