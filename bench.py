@@ -62,7 +62,7 @@ def algorithmic_thread_instr(w: workloads.Workload) -> float:
 def profile_traffic(w: workloads.Workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu summary of
     this workload (profiles/), per launch; None if no capture is committed."""
-    name = {"lattice_N64_2p24": "r01c_lattice_cfg2_dp.md", "realspace_N64_k16_2p22": "r01c_realspace_cfg3.md"}.get(w.name)
+    name = {"lattice_N64_2p24": "r01d_lattice_cfg2.md", "realspace_N64_k16_2p22": "r01d_realspace_cfg3.md"}.get(w.name)
     path = os.path.join(ROOT, "profiles", name) if name else None
     if not path or not os.path.exists(path):
         return None
