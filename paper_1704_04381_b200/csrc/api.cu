@@ -30,6 +30,7 @@ int fail_cuda(cudaError_t e, const char* what)
 struct Scratch {
     Partial*       dev = nullptr;          // [kMaxPartials] block partials
     rosen_summary* summary_dev = nullptr;  // written by finalize_kernel
+    uint32_t*      vb_counter = nullptr;   // virtual-block ticket of the lattice kernel
     rosen_summary* summary_host = nullptr; // pinned mirror
 };
 constexpr int kMaxDevices = 64;
@@ -46,6 +47,7 @@ int get_scratch(Scratch** out)
     if (!s.dev) {
         CK(cudaMalloc(&s.dev, sizeof(Partial) * rosen::kMaxPartials));
         CK(cudaMalloc(&s.summary_dev, sizeof(rosen_summary)));
+        CK(cudaMalloc(&s.vb_counter, sizeof(uint32_t)));
         CK(cudaMallocHost(&s.summary_host, sizeof(rosen_summary)));
     }
     *out = &s;
@@ -164,8 +166,9 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     p.N = N; p.n_chains = n_chains; p.chain_offset = chain_offset;
     p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
     p.ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
-    p.out = st.dev; p.partials = sc->dev;
+    p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
     rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks);
+    CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));
     int grid = 0;
     rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");

@@ -32,6 +32,8 @@ struct LatticeParams {
     Partial*   partials;        // [n_vblocks]
     uint32_t   chunk;           // chains per virtual block (multiple of 256)
     uint32_t   n_vblocks;       // ceil(n_chains / chunk) <= kMaxPartials
+    uint32_t*  vb_counter;      // zeroed before the launch: blocks draw virtual blocks from it (load balance only;
+                                // partials[v] never depends on which block computed it)
 };
 
 struct RealParams {

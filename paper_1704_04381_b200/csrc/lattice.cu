@@ -182,7 +182,12 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
 
     const uint32_t per_thread = p.chunk / blockDim.x;
 
-    for (uint32_t vb = blockIdx.x; vb < p.n_vblocks; vb += gridDim.x) {
+    __shared__ uint32_t vb_ticket;
+    for (;;) {
+        if (threadIdx.x == 0) vb_ticket = atomicAdd(p.vb_counter, 1u);    // dynamic draw: no tail of idle blocks
+        __syncthreads();
+        const uint32_t vb = vb_ticket;      // every thread reads it before the barriers inside block_reduce_store
+        if (vb >= p.n_vblocks) break;
         Partial acc = partial_zero();
         for (uint32_t it = 0; it < per_thread; ++it) {
             const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * blockDim.x + threadIdx.x;
