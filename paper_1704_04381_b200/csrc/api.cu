@@ -206,12 +206,14 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
         p.prefilter2 = r2;
     }
     p.ln_shift = (double)(N - 1) * std::log((double)k_trials);
-    p.out = st.dev; p.partials = sc->dev;
+    p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
+    rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks, 256u);
+    CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));
     int grid = 0;
     rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space kernel launch");
     g_launches += rc;
-    return finish(sc, grid, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
+    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
 }
 
 }  // namespace

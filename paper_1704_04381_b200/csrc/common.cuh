@@ -48,20 +48,22 @@ struct RealParams {
     Partial*   partials;        // [n_vblocks]
     uint32_t   chunk;           // chains per virtual block (multiple of 256)
     uint32_t   n_vblocks;
+    uint32_t*  vb_counter;      // as in LatticeParams
 };
 
 // The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the
 // chain range [v*chunk, (v+1)*chunk) and produces partials[v] with a fixed thread mapping and tree, so
 // the sums depend on (n_chains, N) only -- never on the grid size, occupancy, output variant or GPU.
+// (Real space: chunk >= 256 because one chain occupies a lane group for ~100x longer than a lattice chain.)
 constexpr int kMaxPartials = 8192;
 constexpr uint32_t kMinChunk = 2048;
 
 // chunk = chains per virtual block: >= kMinChunk, a multiple of 256, and large enough for <= kMaxPartials blocks.
-inline void partition_chains(uint64_t n_chains, uint32_t* chunk, uint32_t* n_vblocks)
+inline void partition_chains(uint64_t n_chains, uint32_t* chunk, uint32_t* n_vblocks, uint32_t min_chunk = kMinChunk)
 {
     uint64_t c = (n_chains + kMaxPartials - 1) / kMaxPartials;
     c = (c + 255) / 256 * 256;
-    if (c < kMinChunk) c = kMinChunk;
+    if (c < min_chunk) c = min_chunk;
     *chunk = (uint32_t)c;
     *n_vblocks = (uint32_t)((n_chains + c - 1) / c);
 }

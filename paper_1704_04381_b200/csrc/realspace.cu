@@ -85,14 +85,20 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
     for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
     __syncthreads();
 
+    // Virtual blocks (common.cuh): virtual block vb owns chains [vb*chunk, (vb+1)*chunk); group g of the block takes
+    // chains vb*chunk + it*gpb + g. Blocks draw virtual blocks from a ticket counter, so the grid only balances load.
+    const uint32_t gpb = blockDim.x / G;                     // groups per block; chunk is a multiple of 256 >= gpb
+    const uint32_t iters = p.chunk / gpb;                    // the same for every group of a warp (warp primitives below)
+    __shared__ uint32_t vb_ticket;
+    for (;;) {
+    if (threadIdx.x == 0) vb_ticket = atomicAdd(p.vb_counter, 1u);
+    __syncthreads();
+    const uint32_t vb = vb_ticket;
+    if (vb >= p.n_vblocks) break;
     Partial acc = partial_zero();
-    const uint64_t n_groups = ((uint64_t)gridDim.x * blockDim.x) / G;
-    const uint64_t first = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) / G;
-    // all groups of a warp run the same number of iterations (warp-level primitives below)
-    const uint64_t iters = (p.n_chains + n_groups - 1) / n_groups;
 
-    for (uint64_t it = 0; it < iters; ++it) {
-        const uint64_t idx = first + it * n_groups;
+    for (uint32_t it = 0; it < iters; ++it) {
+        const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * gpb + (uint32_t)group_in_block;
         const bool active = idx < p.n_chains;               // inactive groups compute and discard
         const uint64_t chain = p.chain_offset + idx;
         const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
@@ -248,7 +254,8 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
         __syncwarp();
     }
 
-    block_reduce_store(acc, scratch, p.partials + blockIdx.x);
+    block_reduce_store(acc, scratch, p.partials + vb);
+    }
 }
 
 template <int G, int P, bool DIGEST, bool TRAJ>
@@ -258,8 +265,6 @@ int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    int smem_sm = 0;
-    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
     const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
     int threads = 256;
@@ -270,14 +275,9 @@ int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
-    // variant-independent grid (see lattice.cu): shared-memory / thread limits only
-    per_sm = (int)std::min<size_t>(2048 / threads, (size_t)(smem_sm - 1024) / (smem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    const uint64_t groups_per_block = threads / G;
-    uint64_t want = (p.n_chains + groups_per_block - 1) / groups_per_block;
+    // one resident wave of this variant; the sums do not depend on the grid (virtual blocks)
     uint64_t cap = (uint64_t)n_sm * per_sm;
-    if (cap > (uint64_t)kMaxPartials) cap = kMaxPartials;
-    const int grid = (int)(want < cap ? want : cap);
+    const int grid = (int)(p.n_vblocks < cap ? p.n_vblocks : cap);
     kern<<<grid, threads, smem, stream>>>(p);
     if (cudaGetLastError() != cudaSuccess) return -3;
     *grid_out = grid;
