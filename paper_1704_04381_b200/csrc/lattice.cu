@@ -120,23 +120,31 @@ __device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t 
     "add.s32 u0, t0, -1; add.s32 u1, t1, -1; add.s32 u2, t2, -1; add.s32 u3, t3, -1;\n"                \
     "lop3.b32 t0, t0, u0, nm, 0xE0; lop3.b32 t1, t1, u1, nm, 0xE0; lop3.b32 t2, t2, u2, nm, 0xE0; lop3.b32 t3, t3, u3, nm, 0xE0;\n" \
     "dp4a.u32.u32 t0, t0, on, zr; dp4a.u32.u32 t1, t1, on, zr; dp4a.u32.u32 t2, t2, on, zr; dp4a.u32.u32 t3, t3, on, zr;\n" \
-    "mul.lo.u32 t0, t0, 32; mul.lo.u32 t1, t1, 32; mul.lo.u32 t2, t2, 32; mul.lo.u32 t3, t3, 32;\n"    \
-    "shr.u32 w0, w0, t0; shr.u32 w1, w1, t1; shr.u32 w2, w2, t2; shr.u32 w3, w3, t3;\n"                \
-    "lop3.b32 A, A, w0, w1, 0x96; lop3.b32 A, A, w2, w3, 0x96;\n"
+    "mul.lo.u32 t0, t0, 32; mul.lo.u32 t2, t2, 32;\n"                                                  \
+    "shr.u32 w0, w0, t0; shr.u32 w2, w2, t2;\n"                                                        \
+    "setp.eq.u32 p1, t1, 0; setp.eq.u32 p3, t3, 0;\n"                                                  \
+    "lop3.b32 A, A, w0, w2, 0x96; @p1 xor.b32 A, A, w1; @p3 xor.b32 A, A, w3;\n"
 
 __device__ __forceinline__ uint32_t scan_dpw(uint32_t addr, uint32_t T, uint32_t h)
 {
     uint32_t A;
     asm volatile("{\n"
-        ".reg .pred q;\n"
-        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, cnt, A, nm, on, zr, w0, w1, w2, w3, t0, t1, t2, t3, u0, u1, u2, u3;\n"
+        ".reg .pred q, p1, p3;\n"
+        ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, od, cnt, A, nm, on, zr, w0, w1, w2, w3, t0, t1, t2, t3, u0, u1, u2, u3;\n"
         "mov.u32 ad, %1; mov.u32 cnt, %2; mov.u32 A, 0; mov.u32 nm, 0xFFEFFBFE; mov.u32 on, 0x01010101; mov.u32 zr, 0;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
+        "and.b32 od, cnt, 1;\n"
+        "setp.eq.u32 q, od, 0;\n"
+        "@q bra DPW_EVEN;\n"
+        ROSEN_DPW_CHUNK(a)
+        "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+16];\n"
+        "add.u32 ad, ad, 16; sub.u32 cnt, cnt, 1;\n"
+        "DPW_EVEN:\n"
+        "setp.eq.u32 q, cnt, 0;\n"
+        "@q bra DPW_DONE;\n"
         "DPW_LOOP:\n"
         "ld.shared.v4.b32 {b0, b1, b2, b3}, [ad+16];\n"
         ROSEN_DPW_CHUNK(a)
-        "setp.eq.u32 q, cnt, 1;\n"
-        "@q bra DPW_DONE;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad+32];\n"
         ROSEN_DPW_CHUNK(b)
         "add.u32 ad, ad, 32; sub.u32 cnt, cnt, 2;\n"
