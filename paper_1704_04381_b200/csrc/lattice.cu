@@ -213,6 +213,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
             uint64_t dg = 0xCBF29CE484222325ull;
             uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
 
+#pragma unroll 2
             for (int q = 0; 4 * q < N; ++q) {
                 uint32_t w[4];
                 philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.key0, p.key1, w);   // L1
