@@ -39,7 +39,7 @@ extern "C" {
 
 #define ROSEN_OK        0
 #define ROSEN_EINVAL   (-1)  /* N < 2, n_chains == 0, k_trials outside 1..255, bond_len <= 0, sigma < 0, NaN/inf */
-#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 512, real space 1024)             */
+#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 512, real space 2048)             */
 #define ROSEN_ECUDA    (-3)  /* a CUDA runtime call failed (no device, launch error, ...); see rosen_last_error */
 #define ROSEN_ENOMEM   (-4)  /* staging / workspace allocation failed                                           */
 
@@ -47,7 +47,7 @@ extern "C" {
 #define ROSEN_MEM_HOST   1
 
 #define ROSEN_LATTICE_MAX_N    512
-#define ROSEN_REALSPACE_MAX_N 1024
+#define ROSEN_REALSPACE_MAX_N 2048   /* the paper's longest shared-memory chain, Table 2 */
 
 /*
  * Ensemble summary, Eq. 2 and Eq. 6 (:362). w_c = exp(lnW_c - ln_shift) for a chain

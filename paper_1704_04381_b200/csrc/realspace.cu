@@ -299,7 +299,7 @@ int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kern
 {
     int blocks = (p.k + 1) / 2;   // Philox blocks (trial pairs) per step
     // Long chains: a warp holds 32/G chains of group_bytes(N) each; widen the group (idle lanes own trials >= k)
-    // until one warp's chains fit 24 KB, so that a block of >= 4 warps fits shared memory up to N = 1024.
+    // until one warp's chains fit 24 KB, so that a block of >= 4 warps fits shared memory (N = 2048: one chain per warp, 2 warps per block).
     {
         const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
         int g_mem = 1;

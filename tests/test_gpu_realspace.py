@@ -72,7 +72,7 @@ def test_config5_prefix(R):
     (40, 300, 32, 2.0, 1.7, 9, 0), (31, 300, 33, 1.0, 1.0, 10, 0), (25, 300, 64, 1.0, 1.0, 10, 0),
     (25, 200, 65, 1.0, 0.8, 11, 0), (20, 150, 128, 1.0, 1.0, 11, 0), (18, 100, 129, 1.0, 1.0, 12, 0),
     (12, 100, 255, 1.0, 1.0, 12, 0), (130, 64, 16, 1.0, 1.0, 13, 0), (64, 2000, 16, 1.0, 1.9, 14, 0),
-    (1024, 6, 4, 1.0, 0.6, 15, 0), (1024, 3, 2, 0.5, 0.0, 15, 2),        # ROSEN_REALSPACE_MAX_N
+    (1024, 6, 4, 1.0, 0.6, 15, 0), (1024, 3, 2, 0.5, 0.0, 15, 2), (2048, 3, 3, 1.0, 0.5, 16, 1),   # ROSEN_REALSPACE_MAX_N
 ])
 def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
     check(R, N, n, k, b, sigma, seed, offset)
@@ -104,7 +104,7 @@ def test_error_codes(R):
     bad = [((1, 10, 4, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 0, 1.0, 1.0, 0), R.ROSEN_EINVAL),
            ((8, 10, 256, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, 0.0, 1.0, 0), R.ROSEN_EINVAL),
            ((8, 10, 4, 1.0, -1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, float("nan"), 1.0, 0), R.ROSEN_EINVAL),
-           ((1025, 10, 4, 1.0, 1.0, 0), R.ROSEN_ERANGE)]
+           ((2049, 10, 4, 1.0, 1.0, 0), R.ROSEN_ERANGE)]
     for args, code in bad:
         with pytest.raises(R.RosenError) as e:
             R.rosen_realspace_generate(*args)
