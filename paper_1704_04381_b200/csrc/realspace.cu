@@ -24,12 +24,15 @@ namespace {
 // "rngonsphere" (Alg. 2 line 10) on two Philox words -- DESIGN.md 3.3.
 __device__ __forceinline__ void direction(uint32_t wz, uint32_t wphi, float& ux, float& uy, float& uz)
 {
-    const float z = __fmaf_rn(__uint2float_rn(2u * (wz >> 9) + 1u), 0x1p-23f, -1.0f);
+    // integer -> float through the 2^23 magic number (exact below 2^23; keeps the conversions off the XU pipe).
+    // z: fma(float(q), 2^-22, -(1 - 2^-23)) is the same real number (2q+1) 2^-23 - 1 rounded once, i.e. the same bits.
+    const float qf = __fsub_rn(__uint_as_float(0x4B000000u | (wz >> 9)), 8388608.0f);
+    const float z = __fmaf_rn(qf, 0x1p-22f, -0x1.fffffcp-1f);
     const uint32_t a = wphi >> 8;
     const uint32_t oct = a >> 21;
     const uint32_t f = a & 0x1FFFFFu;
     const uint32_t g = (oct & 1u) ? (0x1FFFFFu - f) : f;
-    const float x = __fmul_rn(__uint2float_rn(2u * g + 1u), 0x1.921fb6p-23f);
+    const float x = __fmul_rn(__fsub_rn(__uint_as_float(0x4B000000u | (2u * g + 1u)), 8388608.0f), 0x1.921fb6p-23f);
     const float x2 = __fmul_rn(x, x);
     float p = __fmaf_rn(x2, 0x1.71de3ap-19f, -0x1.a01a02p-13f);
     p = __fmaf_rn(x2, p, 0x1.111112p-7f);
