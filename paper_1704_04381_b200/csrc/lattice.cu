@@ -7,7 +7,8 @@
 // The scan is the hot loop and is hand-scheduled in PTX. It never compares a key with the six
 // neighbour keys: it classifies w = key_j - h (an integer, because the fields cannot borrow into each other for
 // chains this short) with a byte dot product on the tensor-free IDP.4A path and XOR-accumulates the neighbours'
-// w without predicates -- 5.5 issue slots per key (N <= 64) or 7.5 (N <= 512) instead of 6 half-rate ISETP.
+// w (half of the keys select by a clamped shift, half by a predicate: that balances the alu and fma-heavy pipes)
+// -- about 5.25 issue slots per key (N <= 64) or 7.25 (N <= 512) instead of 6 half-rate ISETP.
 #include <algorithm>
 #include <math_constants.h>
 #include "common.cuh"
@@ -38,7 +39,8 @@ __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 // neighbour and >= 1 otherwise, and w >> (32 d) keeps w or clears it (PTX shr clamps at 32). Every
 // neighbour site holds at most one monomer, so the XOR of {1, -1, 256, -256, 65536, -65536} over the
 // occupied subset decodes uniquely from bits 0,1,8,9,16,17 (table index, build_dp_tables).
-// Per key: IADD, IABS, IDP.4A, IMAD.SHL, SHF, 1/2 LOP3 -- 5.5 issue slots against 8 for the compare scan.
+// Per key: IADD, IABS, IDP.4A, then either IMAD.SHL, SHF, 1/2 LOP3 (keys 0, 2 of a chunk) or ISETP, predicated LOP3
+// (keys 1, 3) -- 5.25 issue slots against 8 for the compare scan.
 // -----------------------------------------------------------------------------------------------------
 struct DpTables {
     uint2    lut[64];   // index = (b0,b1,b8,b9,b16,b17) of the XOR. .x: bits 0-2 = m, bits 4+4i..6+4i = i-th free
@@ -208,7 +210,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
             uint32_t h = kOrigin;
             sts128(ev_addr, h);
             int sx = 0, sy = 0, sz = 0, s2 = 0;
-            uint32_t hist = 0, alive_i = 1u, steps = 0;
+            uint32_t hist = 0, dead = 0;     // dead = step of the first m = 0 (0: alive)
             double lnW_w = 0.0;             // WIDE: running sum (counts can exceed the 8-bit histogram)
             uint64_t dg = 0xCBF29CE484222325ull;
             uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
@@ -233,15 +235,14 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                     const uint32_t m = le.x & 7u;
 
                     // L3
-                    steps += alive_i;
                     if (WIDE) lnW_w += tab->ln_m[m]; else hist += le.y;
-                    if (TRAJ && mrow) mrow[s - 1] = alive_i ? (uint8_t)m : (uint8_t)0;
+                    if (TRAJ && mrow) mrow[s - 1] = dead == 0u ? (uint8_t)m : (uint8_t)0;
 
                     // L4
                     const uint32_t sel = __umulhi(w[k], m);
                     const uint32_t d4 = (le.x >> (4u * sel + 2u)) & 0x1Cu;     // 4 * direction
-                    if (DIGEST) { if (alive_i) dg = digest_fold(dg, m, m ? (d4 >> 2) : 0xFFu); }
-                    alive_i &= min(m, 1u);
+                    if (DIGEST) { if (dead == 0u) dg = digest_fold(dg, m, m ? (d4 >> 2) : 0xFFu); }
+                    dead = (m == 0u && dead == 0u) ? (uint32_t)s : dead;
                     h += lds32(delta_addr + d4);
                     const uint32_t slot = ((k & 1) ? od_addr : ev_addr) + 4u * (uint32_t)(s >> 1);
                     if (((s >> 1) & 3) == 0) sts128(slot, h); else sts32(slot, h);
@@ -259,7 +260,8 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                 }
             }
 
-            const bool alive = alive_i != 0u;
+            const bool alive = dead == 0u;
+            const uint32_t steps = alive ? (uint32_t)(N - 1) : dead;     // attempted steps
             double lnW = tab->ln_m[6];
             lnW += (double)(hist & 255u) * tab->ln_m[2];
             lnW += (double)((hist >> 8) & 255u) * tab->ln_m[3];
