@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
             // ---- R3
             steps += alive ? 1u : 0u;
             lnW += ln_tab[m];
-            if (TRAJ) { if (gl == 0) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
+            if (TRAJ) { if (gl == 0 && p.out.m_seq) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
 
             // ---- R4: the sel-th free trial
             const uint32_t sel = __umulhi(usel, m);
