@@ -39,14 +39,16 @@ extern "C" {
 
 #define ROSEN_OK        0
 #define ROSEN_EINVAL   (-1)  /* N < 2, n_chains == 0, k_trials outside 1..255, bond_len <= 0, sigma < 0, NaN/inf */
-#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 512, real space 2048)             */
+#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 16383, real space 2048)           */
 #define ROSEN_ECUDA    (-3)  /* a CUDA runtime call failed (no device, launch error, ...); see rosen_last_error */
 #define ROSEN_ENOMEM   (-4)  /* staging / workspace allocation failed                                           */
 
 #define ROSEN_MEM_DEVICE 0
 #define ROSEN_MEM_HOST   1
 
-#define ROSEN_LATTICE_MAX_N    512
+#define ROSEN_LATTICE_SCAN_MAX_N 512  /* up to here: chain in shared memory, parity-split scan (lattice.cu)          */
+#define ROSEN_LATTICE_MAX_N  16383   /* beyond: per-chain hash set in HBM (lattice_hash.cu), the range of the paper's
+                                        "global-memory version", Table 1 PAPER.md:282-288 (N = 100 ... 10000)        */
 #define ROSEN_REALSPACE_MAX_N 2048   /* the paper's longest shared-memory chain, Table 2 */
 
 /*
@@ -59,7 +61,8 @@ typedef struct rosen_summary {
     uint64_t n_chains;            /* chains attempted                                                  */
     uint64_t n_dead;              /* chains that hit m_s = 0                                           */
     uint64_t n_steps_attempted;   /* sum over chains of growth steps attempted (= monomer-steps)       */
-    double   ln_shift;            /* L: lattice ln6 + (N-2) ln5, real space (N-1) ln k                 */
+    double   ln_shift;            /* L: lattice ln6 + (N-2) ln5 (N <= 512) or ln6 + (N-2) ln 4.684     */
+                                  /*    (N > 512, reading A16); real space (N-1) ln k        */
     double   sum_w, sum_w_ree2, sum_w_rg2, sum_w2;
     double   mean_ree2;           /* sum_w_ree2 / sum_w   : W-weighted <R_ee^2>                        */
     double   mean_rg2;            /* sum_w_rg2 / sum_w    : W-weighted <R_g^2>                         */
@@ -91,7 +94,9 @@ typedef struct rosen_outputs {
  * r_{s-1}, in the order +x,-x,+y,-y,+z,-z, are tested against all earlier monomers, m_s = number
  * of free ones, lnW += ln m_s, and the ((u_s * m_s) >> 32)-th free neighbour is taken, u_s being
  * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
- * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N.
+ * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N > ROSEN_LATTICE_SCAN_MAX_N the library keeps device
+ * workspace (at most 8 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
+ * rosen_workspace_release(); the results do not depend on which kernel ran.
  */
 ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
                            const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
@@ -159,8 +164,13 @@ typedef struct rosen_fit {
 ROSEN_API int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double* ln_mean_W,
                                   int32_t count, int32_t use_steps, rosen_fit* fit);
 
-/* Bytes of device scratch the library keeps per device for block partials (informational). */
+/* Bytes of device scratch the library currently keeps on the current device: block partials, plus the
+ * long-chain workspace of the lattice call if one was made (informational). */
 ROSEN_API size_t rosen_workspace_bytes(void);
+
+/* Free the long-chain workspace of the current device (synchronises the device). Always ROSEN_OK; the next
+ * long-chain call allocates it again. */
+ROSEN_API int rosen_workspace_release(void);
 
 /*
  * Number of kernel launches the last generate/dump call on this thread enqueued, and the name of

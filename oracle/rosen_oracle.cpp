@@ -150,7 +150,10 @@ int oracle_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_
                             const oracle_outputs* out, oracle_summary* summary)
 {
     if (N < 2 || n_chains == 0) return -1;
-    const double L = std::log(6.0) + (double)(N - 2) * std::log(5.0);     // max possible lnW
+    // L: the largest possible lnW for N <= 512; beyond that exp(lnW - L) would underflow fp64 (lnW - L ~ -0.065 N),
+    // so long chains are shifted by the paper's growth constant mu = 4.684 (Table 4) instead
+    // (reading A16). L is a constant of N: it cancels in every ratio of Eq. 2 and is added back in Eq. 6.
+    const double L = std::log(6.0) + (double)(N - 2) * std::log(N <= 512 ? 5.0 : 4.684);
     std::vector<int32_t> r((size_t)N * 3);
     Comp sw, swr, swg, sw2;
     uint64_t n_dead = 0, n_steps = 0, dxor = 0, dsum = 0;

@@ -82,6 +82,8 @@ def load_library() -> C.CDLL:
     L.rosen_summary_merge.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
     L.rosen_workspace_bytes.restype = C.c_size_t
+    L.rosen_workspace_release.argtypes = []
+    L.rosen_workspace_release.restype = C.c_int
     L.rosen_last_launch_count.argtypes = []
     L.rosen_last_launch_count.restype = i32
     for name in ("rosen_last_kernel_name", "rosen_last_error", "rosen_version"):
@@ -266,6 +268,10 @@ def rosen_fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> Dict
 
 def rosen_workspace_bytes() -> int:
     return int(load_library().rosen_workspace_bytes())
+
+
+def rosen_workspace_release() -> int:
+    return int(load_library().rosen_workspace_release())
 
 
 def rosen_last_launch_count() -> int:

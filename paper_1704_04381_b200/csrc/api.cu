@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -32,7 +33,12 @@ struct Scratch {
     rosen_summary* summary_dev = nullptr;  // written by finalize_kernel
     uint32_t*      vb_counter = nullptr;   // virtual-block ticket of the lattice kernel
     rosen_summary* summary_host = nullptr; // pinned mirror
+    // long-chain lattice path (lattice_hash.cu): grown on demand, kept until rosen_workspace_release()
+    void*          hash_tables = nullptr;  size_t hash_tables_bytes = 0;
+    void*          hash_rec = nullptr;     size_t hash_rec_bytes = 0;
+    unsigned long long* hash_ticket = nullptr;
 };
+constexpr size_t kHashTableCap = (size_t)8 << 30;   // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
 Scratch g_scratch[kMaxDevices];
 std::mutex g_mutex;
@@ -52,6 +58,25 @@ int get_scratch(Scratch** out)
     }
     *out = &s;
     return ROSEN_OK;
+}
+
+int grow(void** ptr, size_t* have, size_t need)
+{
+    if (*have >= need) return ROSEN_OK;
+    if (*ptr) { cudaDeviceSynchronize(); cudaFree(*ptr); *ptr = nullptr; *have = 0; }
+    cudaError_t e = cudaMalloc(ptr, need);
+    if (e != cudaSuccess) { fail_cuda(e, "cudaMalloc(long-chain workspace)"); *ptr = nullptr; return ROSEN_ENOMEM; }
+    *have = need;
+    return ROSEN_OK;
+}
+
+// chain length from which the lattice call uses the hash-set kernel; ROSEN_LATTICE_HASH_MIN_N overrides it
+// (tests run the hash kernel on short chains too, where the enumeration pins apply)
+int32_t hash_min_n()
+{
+    const char* e = std::getenv("ROSEN_LATTICE_HASH_MIN_N");
+    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_LATTICE_MAX_N) return (int32_t)v; }
+    return ROSEN_LATTICE_SCAN_MAX_N + 1;
 }
 
 struct Sizes { size_t lnW, alive, m_seq, digest, conf, ree2, rg2; };
@@ -162,10 +187,45 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     Staging st;
     if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
 
+    // largest possible lnW up to N = 512; beyond, the paper's mu = 4.684 (Table 4) keeps exp(lnW - L) inside
+    // fp64 (reading A16)
+    const double ln_shift = std::log(6.0) + (double)(N - 2) * std::log(N <= ROSEN_LATTICE_SCAN_MAX_N ? 5.0 : 4.684);
+    if (N >= hash_min_n()) {
+        // long chains: per-chain hash map cube -> occupancy bitmap in HBM (lattice_hash.cu)
+        rosen::HashParams hp{};
+        hp.N = N; hp.n_chains = n_chains; hp.chain_offset = chain_offset;
+        hp.key0 = (uint32_t)seed; hp.key1 = (uint32_t)(seed >> 32);
+        hp.ln_shift = ln_shift; hp.out = st.dev; hp.partials = sc->dev;
+        rosen::partition_chains(n_chains, &hp.chunk, &hp.n_vblocks, 256u);
+        hp.log2_entries = rosen::hash_log2_entries(N);
+        const size_t table_bytes = ((size_t)16) << hp.log2_entries;      // 16-byte entries
+        int max_threads = 0;
+        if (rosen::hash_max_threads(&max_threads) < 0) return fail_cuda(cudaGetLastError(), "device query");
+        uint64_t threads = (n_chains + 255) / 256 * 256;
+        if (threads > (uint64_t)max_threads) threads = (uint64_t)max_threads;
+        const uint64_t by_mem = kHashTableCap / table_bytes / 256 * 256;
+        if (threads > by_mem) threads = by_mem;
+        {
+            std::lock_guard<std::mutex> lock(g_mutex);
+            if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, threads * table_bytes))) return rc;
+            if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
+            if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
+        }
+        hp.tables = static_cast<uint64_t*>(sc->hash_tables);
+        hp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
+        hp.ticket = sc->hash_ticket;
+        CK(cudaMemsetAsync(hp.tables, 0, threads * table_bytes, stream));      // generation 0 = empty everywhere
+        CK(cudaMemsetAsync(hp.ticket, 0, sizeof(unsigned long long), stream));
+        rc = rosen::launch_lattice_hash(hp, (int)threads, stream, &g_kernel);
+        if (rc < 0) return fail_cuda(cudaGetLastError(), "lattice hash kernel launch");
+        g_launches += rc;
+        return finish(sc, (int)hp.n_vblocks, n_chains, ln_shift, outputs, z, st, summary, summary_dev, stream);
+    }
+
     rosen::LatticeParams p{};
     p.N = N; p.n_chains = n_chains; p.chain_offset = chain_offset;
     p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
-    p.ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
+    p.ln_shift = ln_shift;
     p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
     rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks);
     CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));
@@ -328,7 +388,30 @@ int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double*
     return ROSEN_OK;
 }
 
-size_t rosen_workspace_bytes(void) { return sizeof(Partial) * rosen::kMaxPartials + sizeof(rosen_summary); }
+size_t rosen_workspace_bytes(void)
+{
+    size_t b = sizeof(Partial) * rosen::kMaxPartials + sizeof(rosen_summary);
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices) {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        b += g_scratch[dev].hash_tables_bytes + g_scratch[dev].hash_rec_bytes;
+    } else {
+        cudaGetLastError();
+    }
+    return b;
+}
+
+int rosen_workspace_release(void)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return ROSEN_OK; }   // nothing was ever allocated
+    std::lock_guard<std::mutex> lock(g_mutex);
+    Scratch& s = g_scratch[dev];
+    if (s.hash_tables || s.hash_rec) cudaDeviceSynchronize();
+    if (s.hash_tables) { cudaFree(s.hash_tables); s.hash_tables = nullptr; s.hash_tables_bytes = 0; }
+    if (s.hash_rec) { cudaFree(s.hash_rec); s.hash_rec = nullptr; s.hash_rec_bytes = 0; }
+    return ROSEN_OK;
+}
 int32_t rosen_last_launch_count(void) { return g_launches; }
 const char* rosen_last_kernel_name(void) { return g_kernel; }
 

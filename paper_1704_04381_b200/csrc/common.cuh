@@ -51,6 +51,29 @@ struct RealParams {
     uint32_t*  vb_counter;      // as in LatticeParams
 };
 
+// Long-chain lattice path (lattice_hash.cu): one fixed-size record per chain, reduced afterwards in a fixed order.
+struct ChainRecord {
+    double   lnW, ree2, rg2;    // -inf / 0 / 0 for a dead chain
+    uint32_t steps, alive;      // attempted steps; 1 = reached N monomers
+    uint64_t digest;
+};
+
+struct HashParams {
+    int32_t    N;
+    uint64_t   n_chains;
+    uint64_t   chain_offset;
+    uint32_t   key0, key1;
+    double     ln_shift;
+    DevOutputs out;
+    Partial*   partials;        // [n_vblocks]
+    uint32_t   chunk;           // chains per virtual block (multiple of 256)
+    uint32_t   n_vblocks;
+    ChainRecord* rec;           // [n_chains]
+    uint64_t*  tables;          // [launched threads][1 << log2_entries] 16-byte entries, zeroed before the launch
+    uint32_t   log2_entries;    // entries per chain table (power of two >= N + 1)
+    unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
+};
+
 // The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the
 // chain range [v*chunk, (v+1)*chunk) and produces partials[v] with a fixed thread mapping and tree, so
 // the sums depend on (n_chains, N) only -- never on the grid size, occupancy, output variant or GPU.
@@ -71,6 +94,11 @@ inline void partition_chains(uint64_t n_chains, uint32_t* chunk, uint32_t* n_vbl
 // launchers (lattice.cu / realspace.cu / reduce.cu). Return the number of kernels launched or
 // a negative ROSEN_E* code; *kernel_name receives a static string naming the variant chosen.
 int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
+// lattice_hash.cu: table geometry for chain length N, resident thread capacity of the device, launch (generation
+// kernel over n_threads = multiple of 256 threads, then the per-record first reduction pass).
+uint32_t hash_log2_entries(int32_t N);
+int hash_max_threads(int* threads_out);
+int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift,
                     void* summary_dev, cudaStream_t stream);   // summary_dev: rosen_summary* in device memory

@@ -1,0 +1,275 @@
+// lattice_hash.cu -- cubic-lattice Rosenbluth generation for LONG chains (512 < N <= 16383), the range of the
+// paper's "global-memory version" (Table 1; Fig. 2b, :296) and of its longest shared-memory
+// rows (N = 1024, 2048, :280-281). Same steps L0-L5 and the same decisions as lattice.cu, but
+// the occupancy scan of Alg. 1 lines 13-17, which costs O(s) per step, is replaced by an
+// exact per-chain hash map of occupied sites in global memory: O(N) per chain instead of O(N^2)
+// ("a per-chain hash set would make it ~5 probes/step").
+//
+// Layout. One thread grows one chain. Space is cut into 4 x 4 x 4 cubes; the chain's table maps a
+// cube to the 64-bit occupancy bitmap of its sites. An entry is 16 bytes:
+//   .x  bits 0..38   cube key (cx+2^12) | (cy+2^12) << 13 | (cz+2^12) << 26, c = coordinate >> 2 (floor)
+//       bits 39..63  the thread's chain generation (1, 2, ...): an entry whose generation differs from the current
+//                    chain's is EMPTY, so tables are never cleared between chains (one memset per launch)
+//   .y  bit (x&3) | (y&3) << 2 | (z&3) << 4 set = site occupied
+// Tables are open-addressed (Fibonacci hash of the cube key, linear probing, no deletions) with a power of two
+// >= N+1 entries: a chain of N monomers touches at most N cubes, so a probe always ends at an empty entry.
+// The growth point's own cube lives in registers (bitmap + entry index); of the six neighbour sites only those
+// across a cube face need memory: at most three look-ups per step, 1.5 on average, against five for a per-site set,
+// and the insert is a 16-byte store to an entry that is already known.
+//
+// Scheduling. Chains of this length die often (attrition 20 % at N = 1024, 93 % at N = 10000) and run for very
+// different times, so lanes draw chain indices from a global ticket one by one and every warp iteration is one
+// growth step of each lane's current chain -- no lane waits for its neighbours' chains. Because that order is
+// timing dependent, the kernel only writes one fixed-size record per chain; the ensemble sums are formed afterwards
+// by reduce_records_kernel over virtual blocks in a fixed order (deterministic, grid independent, no float
+// atomics), which also writes the optional per-chain outputs, coalesced.
+//
+// Roofline: random sector traffic to HBM/L2, not issue slots (DESIGN.md 5.5 / 6).
+#include <cstdlib>
+#include <math_constants.h>
+#include "common.cuh"
+#include "philox.cuh"
+#include "reduce.cuh"
+
+namespace rosen {
+
+namespace {
+
+constexpr int      kCubeField = 13;
+constexpr uint64_t kCubeBias = 1ull << (kCubeField - 1);
+constexpr uint64_t kOriginCube = kCubeBias | (kCubeBias << kCubeField) | (kCubeBias << (2 * kCubeField));
+constexpr int      kGenShift = 3 * kCubeField;                       // 39
+constexpr uint32_t kGenMax = (1u << (64 - kGenShift)) - 1u;
+
+__device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t choice)
+{
+    return (h ^ (uint64_t)(m | (choice << 8))) * 0x100000001B3ull;
+}
+
+__device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t shift)
+{
+    return (uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> shift);
+}
+
+__device__ __forceinline__ ulonglong2 load_entry(const ulonglong2* table, uint32_t slot) { return table[slot]; }
+
+// three-way select by axis
+template <typename T> __device__ __forceinline__ T pick(uint32_t a, T v0, T v1, T v2) { return a == 0u ? v0 : (a == 1u ? v1 : v2); }
+
+template <bool TRAJ>
+__global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p)
+{
+    __shared__ double ln_m[8];
+    if (threadIdx.x < 8) ln_m[threadIdx.x] = threadIdx.x == 0 ? -CUDART_INF : log((double)threadIdx.x);
+    __syncthreads();
+
+    const int N = p.N;
+    const uint32_t shift = 64u - p.log2_entries, mask = (1u << p.log2_entries) - 1u;
+    const uint64_t entries = 1ull << p.log2_entries;
+    ulonglong2* table = reinterpret_cast<ulonglong2*>(p.tables) + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * entries;
+    uint32_t gen = 0;
+
+    // per-lane state of the chain being grown; s == 0: the lane needs a new chain
+    uint64_t idx = 0, tag = 0, dg = 0;
+    uint64_t cube = 0, bits = 0;            // the growth point's cube: key and occupancy bitmap (register copy of its entry)
+    uint32_t slot = 0, l = 0;               // its entry index; local site index of the growth point inside it
+    uint32_t c_lo = 0, c_hi = 0, w[4] = {0u, 0u, 0u, 0u};
+    int s = 0, x = 0, y = 0, z = 0, sx = 0, sy = 0, sz = 0;
+    long long s2 = 0;
+    double lnW = 0.0;
+    uint8_t* mrow = nullptr;
+    int32_t* crow = nullptr;
+
+    // One iteration = one growth step of every lane's current chain. A lane whose chain ended (full length or dead
+    // end) writes its record and draws the next chain in the same iteration, so no lane idles while its neighbours'
+    // chains are still growing.
+    for (;;) {
+        if (s == 0) {
+            // ---- draw the next chain (timing dependent; results are not: a record is a function of the chain id)
+            idx = atomicAdd(p.ticket, 1ull);
+            if (idx >= p.n_chains) break;
+            const uint64_t chain = p.chain_offset + idx;
+            c_lo = (uint32_t)chain; c_hi = (uint32_t)(chain >> 32);
+            if (++gen > kGenMax) {     // generation counter wrapped: clear the table once and start over
+                for (uint64_t i = 0; i < entries; ++i) table[i] = make_ulonglong2(0ull, 0ull);
+                gen = 1u;
+            }
+            tag = (uint64_t)gen << kGenShift;
+            // ---- L0: r_0 = origin; every entry is empty for a new generation, so the origin's cube takes its home slot
+            cube = kOriginCube; bits = 1ull; l = 0u;
+            slot = slot_of(cube, shift);
+            table[slot] = make_ulonglong2(cube | tag, bits);
+            x = y = z = sx = sy = sz = 0; s2 = 0; lnW = 0.0; s = 1;
+            dg = 0xCBF29CE484222325ull;
+            philox4x32_10(c_lo, c_hi, 0u, 0u, p.key0, p.key1, w);             // L1, block of steps 1..3
+            if (TRAJ) {
+                mrow = p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
+                crow = p.out.conf ? reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3 : nullptr;
+                if (crow) { crow[0] = 0; crow[1] = 0; crow[2] = 0; }
+            }
+        } else if ((s & 3) == 0) {
+            philox4x32_10(c_lo, c_hi, (uint32_t)(s >> 2), 0u, p.key0, p.key1, w);   // L1
+        }
+
+        // ---- L2. Per axis at most one neighbour site lies across a cube face (local coordinate 0 or 3): fetch that
+        // cube's bitmap (all first probes in flight together); the other neighbours are bits of the register bitmap.
+        uint64_t nkey[3], nbits[3];
+        uint32_t nslot[3], nl[3];
+        bool need[3];
+        ulonglong2 first[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const uint32_t la = (l >> (2 * a)) & 3u;
+            const bool up = la == 3u;
+            need[a] = up || la == 0u;
+            nkey[a] = up ? cube + (1ull << (kCubeField * a)) : cube - (1ull << (kCubeField * a));
+            nl[a] = up ? l - (3u << (2 * a)) : l + (3u << (2 * a));
+            nslot[a] = slot_of(nkey[a], shift);
+            first[a] = make_ulonglong2(0ull, 0ull);
+            if (need[a]) first[a] = load_entry(table, nslot[a]);
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            nbits[a] = 0ull;
+            if (need[a]) {
+                ulonglong2 e = first[a];
+                for (;;) {
+                    if ((uint32_t)(e.x >> kGenShift) != gen) break;                    // empty: cube not visited yet; nslot = where it would go
+                    if (e.x == (nkey[a] | tag)) { nbits[a] = e.y; break; }
+                    nslot[a] = (nslot[a] + 1u) & mask;
+                    e = load_entry(table, nslot[a]);
+                }
+            }
+        }
+        uint32_t occ = 0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const uint32_t la = (l >> (2 * a)) & 3u;
+            const uint32_t in_up = (uint32_t)(bits >> ((l + (1u << (2 * a))) & 63u)) & 1u;
+            const uint32_t in_dn = (uint32_t)(bits >> ((l - (1u << (2 * a))) & 63u)) & 1u;
+            const uint32_t out = (uint32_t)(nbits[a] >> (nl[a] & 63u)) & 1u;
+            occ |= (la == 3u ? out : in_up) << (2 * a);             // +axis
+            occ |= (la == 0u ? out : in_dn) << (2 * a + 1);         // -axis
+        }
+        const uint32_t m = 6u - (uint32_t)__popc(occ);
+        if (TRAJ && mrow) mrow[s - 1] = (uint8_t)m;
+
+        bool done;
+        if (m == 0u) {
+            // ---- L3: dead end (W = 0, chain kept; reading A6)
+            dg = digest_fold(dg, 0u, 0xFFu);
+            done = true;
+        } else {
+            lnW += ln_m[m];
+            // ---- L4
+            const uint32_t u = (s & 2) ? ((s & 1) ? w[3] : w[2]) : ((s & 1) ? w[1] : w[0]);
+            const uint32_t sel = __umulhi(u, m);
+            const uint32_t d = __fns(~occ & 63u, 0u, (int)sel + 1);       // sel-th free direction in the order +x,-x,+y,-y,+z,-z
+            dg = digest_fold(dg, m, d);
+            const uint32_t a = d >> 1;
+            const bool up = (d & 1u) == 0u;
+            const uint32_t la = (l >> (2u * a)) & 3u;
+            if (up ? la == 3u : la == 0u) {          // across a cube face: that cube's entry becomes the register copy
+                cube = pick(a, nkey[0], nkey[1], nkey[2]);
+                slot = pick(a, nslot[0], nslot[1], nslot[2]);
+                l = pick(a, nl[0], nl[1], nl[2]);
+                bits = pick(a, nbits[0], nbits[1], nbits[2]);
+            } else {
+                l = up ? l + (1u << (2u * a)) : l - (1u << (2u * a));
+            }
+            bits |= 1ull << l;
+            table[slot] = make_ulonglong2(cube | tag, bits);              // insert r_s (write-through; L2 absorbs repeats)
+            const int sg = up ? 1 : -1;
+            x += a == 0u ? sg : 0; y += a == 1u ? sg : 0; z += a == 2u ? sg : 0;
+            if (TRAJ && crow) { crow[3 * s + 0] = x; crow[3 * s + 1] = y; crow[3 * s + 2] = z; }
+            // ---- L5
+            sx += x; sy += y; sz += z; s2 += (long long)(x * x + y * y + z * z);
+            ++s;
+            done = s == N;
+        }
+
+        if (done) {
+            const bool alive = m != 0u;
+            if (TRAJ && !alive) {      // zero-fill from the death step on (reading A13); m_seq[s-1] = 0 is already there
+                if (mrow) for (int q = s; q < N - 1; ++q) mrow[q] = 0;
+                if (crow) for (int q = 3 * s; q < 3 * N; ++q) crow[q] = 0;
+            }
+            ChainRecord r;
+            r.lnW = alive ? lnW : -CUDART_INF;
+            r.ree2 = 0.0; r.rg2 = 0.0;
+            if (alive) {
+                r.ree2 = (double)((long long)x * x + (long long)y * y + (long long)z * z);
+                const long long num = (long long)N * s2 - ((long long)sx * sx + (long long)sy * sy + (long long)sz * sz);
+                r.rg2 = (double)num / ((double)N * (double)N);
+            }
+            r.steps = alive ? (uint32_t)(N - 1) : (uint32_t)s;     // attempted steps
+            r.alive = alive ? 1u : 0u;
+            r.digest = dg;
+            p.rec[idx] = r;
+            s = 0;
+        }
+    }
+}
+
+// E1, first pass, for kernels that write per-chain records: virtual block v sums the chains [v*chunk, (v+1)*chunk)
+// with the thread mapping and tree of the generation kernels (thread t takes v*chunk + it*256 + t, it ascending).
+__global__ void __launch_bounds__(256) reduce_records_kernel(const ChainRecord* __restrict__ rec, uint64_t n_chains, uint32_t chunk,
+                                                             double ln_shift, DevOutputs out, Partial* partials)
+{
+    __shared__ Partial scratch[8];
+    const uint32_t vb = blockIdx.x;
+    Partial acc = partial_zero();
+    for (uint32_t it = 0; it < chunk / 256u; ++it) {
+        const uint64_t idx = (uint64_t)vb * chunk + (uint64_t)it * 256u + threadIdx.x;
+        if (idx >= n_chains) break;
+        const ChainRecord r = rec[idx];
+        const bool alive = r.alive != 0u;
+        const double wgt = alive ? exp(r.lnW - ln_shift) : 0.0;
+        acc.sum_w += wgt; acc.sum_w_ree2 += wgt * r.ree2; acc.sum_w_rg2 += wgt * r.rg2; acc.sum_w2 += wgt * wgt;
+        acc.n_dead += alive ? 0u : 1u; acc.n_steps += r.steps;
+        if (out.digest) { acc.digest_xor ^= r.digest; acc.digest_sum += r.digest; out.digest[idx] = r.digest; }
+        if (out.lnW) out.lnW[idx] = r.lnW;
+        if (out.alive) out.alive[idx] = alive ? 1 : 0;
+        if (out.ree2) out.ree2[idx] = r.ree2;
+        if (out.rg2) out.rg2[idx] = r.rg2;
+    }
+    block_reduce_store(acc, scratch, partials + vb);
+}
+
+}  // namespace
+
+uint32_t hash_log2_entries(int32_t N)
+{
+    uint32_t lg = 2;                                   // entries = 1 << lg >= N + 1 > cubes one chain can touch
+    while ((1ull << lg) < (uint64_t)N + 1ull) ++lg;
+    return lg;
+}
+
+int hash_max_threads(int* threads_out)
+{
+    int dev = 0, n_sm = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+    // the traj variant has the larger register footprint: size the tables for the plain one, which every launch may use
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lattice_hash_kernel<false>, 256, 0) != cudaSuccess || per_sm < 1) return -3;
+    if (const char* e = std::getenv("ROSEN_HASH_BLOCKS_PER_SM")) {     // tuning knob (results do not depend on it)
+        const int v = std::atoi(e);
+        if (v >= 1 && v < per_sm) per_sm = v;
+    }
+    *threads_out = n_sm * per_sm * 256;
+    return 0;
+}
+
+int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name)
+{
+    const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
+    const int grid = n_threads / 256;
+    if (traj) { *kernel_name = "lattice_hash_kernel<traj>"; lattice_hash_kernel<true><<<grid, 256, 0, stream>>>(p); }
+    else      { *kernel_name = "lattice_hash_kernel";       lattice_hash_kernel<false><<<grid, 256, 0, stream>>>(p); }
+    if (cudaGetLastError() != cudaSuccess) return -3;
+    reduce_records_kernel<<<p.n_vblocks, 256, 0, stream>>>(p.rec, p.n_chains, p.chunk, p.ln_shift, p.out, p.partials);
+    if (cudaGetLastError() != cudaSuccess) return -3;
+    return 2;
+}
+
+}  // namespace rosen

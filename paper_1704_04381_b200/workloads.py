@@ -35,7 +35,13 @@ CONFIG_4_N: Tuple[int, ...] = (8, 16, 32, 64, 128, 256)
 CONFIG_4 = tuple(Workload(f"lattice_sweep_N{N}_2p24", "lattice", N, 1 << 24, 11) for N in CONFIG_4_N)
 CONFIG_5 = Workload("realspace_N256_k64_2p20_dump", "realspace", 256, 1 << 20, 13, 64, 1.0, 0.8, dump=True)
 
-CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5)}
+# Beyond BASELINE.json: the long lattice chains of the paper's Table 1,
+# N = 1024 / 2048 of the shared-memory rows and N = 10000, the longest "global-memory version" row.
+LONG_LATTICE = (Workload("lattice_long_N1024_2p20", "lattice", 1024, 1 << 20, 17),
+                Workload("lattice_long_N2048_2p19", "lattice", 2048, 1 << 19, 17),
+                Workload("lattice_long_N10000_2p17", "lattice", 10000, 1 << 17, 17))
+
+CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5, *LONG_LATTICE)}
 
 
 def shard(n_chains: int, rank: int, world: int) -> Tuple[int, int]:

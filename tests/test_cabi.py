@@ -26,7 +26,7 @@ def declared_symbols():
 def test_every_declared_symbol_is_exported(R):
     from paper_1704_04381_b200 import binding
     names = declared_symbols()
-    assert len(names) == 14 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
+    assert len(names) == 15 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
     lib = ctypes.CDLL(binding.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), n
@@ -43,6 +43,7 @@ def test_host_only_entry_points(R):
     assert "sm_100a" in R.rosen_version()
     assert R.rosen_strerror(R.ROSEN_OK) == "success" and "invalid" in R.rosen_strerror(R.ROSEN_EINVAL)
     assert R.rosen_workspace_bytes() >= 8192 * 64
+    assert R.rosen_workspace_release() == R.ROSEN_OK      # nothing allocated yet: still OK
     a = dict(n_chains=10, n_dead=1, n_steps_attempted=90, ln_shift=2.0, sum_w=4.0, sum_w_ree2=8.0, sum_w_rg2=2.0,
              sum_w2=3.0, mean_ree2=2.0, mean_rg2=0.5, attrition=0.1, ln_mean_W=0.0, digest_xor=5, digest_sum=7)
     b = dict(a, n_chains=30, n_dead=0, sum_w=12.0, sum_w_ree2=12.0, digest_xor=6, digest_sum=2 ** 64 - 3)

@@ -70,6 +70,75 @@ def test_shapes_ragged_and_edges(R, N, n_chains, seed, offset):
     compare_summary(s, o.summary)
 
 
+# Long chains (N > ROSEN_LATTICE_SCAN_MAX_N = 512): the hash-set kernel of lattice_hash.cu, the range of the paper's
+# "global-memory version" (Table 1). Same bit-exact bar as the scan kernel. Sizes keep the oracle's
+# O(N^2) scan to seconds; N = 1366 is the first length of the 4096-slot table, 1365 the fullest 2048-slot one.
+@pytest.mark.parametrize("N,n_chains,seed,offset", [
+    (513, 1000, 14, 0), (1024, 777, 15, 5), (1365, 300, 16, 0), (1366, 300, 16, 0), (2048, 400, 17, 1 << 33),
+    (4096, 257, 18, 0), (10000, 200, 19, 0), (16383, 100, 20, 0),
+])
+def test_long_chains_hash_kernel(R, N, n_chains, seed, offset):
+    s, t = R.rosen_lattice_generate(N, n_chains, seed, chain_offset=offset, outputs=ALL)
+    assert "lattice_hash_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 3
+    o = oracle.lattice_generate(N, n_chains, seed, chain_offset=offset)
+    compare_per_chain(t, o, N)
+    compare_summary(s, o.summary)
+    s2, _ = R.rosen_lattice_generate(N, n_chains, seed, chain_offset=offset)          # summary-only variant
+    for k in s:
+        if not k.startswith("digest"):
+            assert s[k] == s2[k], k
+
+
+def test_hash_kernel_equals_scan_kernel_on_short_chains(R, monkeypatch):
+    """ROSEN_LATTICE_HASH_MIN_N routes short chains through the hash kernel: it must reproduce the scan kernel
+    (and with it the oracle and its enumeration pins) bit for bit, per chain and in the ensemble sums, with
+    many chains per lane (table generations) and more chains than resident threads."""
+    import torch
+    for N, n, seed in [(16, 1 << 16, 1), (64, 400000, 7), (200, 30011, 3)]:
+        monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N", raising=False)
+        s_scan, t_scan = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
+        assert "lattice_dp_kernel" in R.rosen_last_kernel_name()
+        monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "2")
+        s_hash, t_hash = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
+        assert "lattice_hash_kernel" in R.rosen_last_kernel_name()
+        for k in ALL:
+            if k == "lnW":      # N <= 64: the scan kernel sums an m histogram, the hash kernel adds step by step
+                assert torch.equal(torch.isinf(t_scan[k]), torch.isinf(t_hash[k]))
+                assert torch.allclose(t_scan[k], t_hash[k], rtol=REL, atol=0.0), (N, k)
+            else:
+                assert torch.equal(t_scan[k], t_hash[k]), (N, k)
+        for k in ("n_chains", "n_dead", "n_steps_attempted", "digest_xor", "digest_sum"):
+            assert s_scan[k] == s_hash[k], k
+        for k in ("sum_w", "sum_w_ree2", "sum_w_rg2", "sum_w2", "mean_ree2", "mean_rg2", "ln_mean_W"):
+            assert math.isclose(s_scan[k], s_hash[k], rel_tol=REL), k
+    monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N", raising=False)
+    assert R.rosen_workspace_bytes() > (1 << 20)
+    assert R.rosen_workspace_release() == R.ROSEN_OK
+
+
+def test_long_chain_properties_at_bench_size(R):
+    """N = 1024, 2^18 chains in the launch configuration bench.py --workload lattice_long times: invariants that
+    hold at any size plus sampled chains recomputed one by one by the oracle (chain_offset sub-ranges)."""
+    import torch
+    N, n, seed = 1024, 1 << 18, 23
+    s, t = R.rosen_lattice_generate(N, n, seed, outputs=("lnW", "alive", "ree2", "rg2", "digest"))
+    alive = t["alive"].bool()
+    assert s["n_dead"] == int((~alive).sum()) and 0.1 < s["attrition"] < 0.35
+    assert bool(torch.isinf(t["lnW"][~alive]).all()) and bool((t["ree2"][~alive] == 0).all())
+    L = s["ln_shift"]
+    assert bool((t["lnW"][alive] <= math.log(6.0) + (N - 2) * math.log(5.0) + 1e-9).all()) and abs(L - (math.log(6.0) + (N - 2) * math.log(4.684))) < 1e-9 and bool((t["ree2"][alive] <= (N - 1) ** 2).all())
+    assert bool((t["ree2"][alive] % 2 == (N - 1) % 2).all())           # bipartite lattice: parity of |r|^2 = parity of the step count
+    for off in (0, 77777, n - 3):
+        o = oracle.lattice_generate(N, 3, seed, chain_offset=off)
+        assert np.array_equal(t["digest"][off:off + 3].cpu().numpy().view(np.uint64), o.digest)
+        assert np.array_equal(t["ree2"][off:off + 3].cpu().numpy(), o.ree2)
+        assert np.allclose(t["lnW"][off:off + 3].cpu().numpy(), o.lnW, rtol=REL, atol=0)
+    s2, _ = R.rosen_lattice_generate(N, n, seed)
+    for k in s:
+        if not k.startswith("digest"):
+            assert s[k] == s2[k], k
+
+
 def test_summary_only_variant_is_bit_identical_and_deterministic(R):
     N, n, seed = 64, 100003, 7
     s0, _ = R.rosen_lattice_generate(N, n, seed)
@@ -117,7 +186,7 @@ def test_chain_offset_subrange_and_merge(R):
 
 
 def test_error_codes(R):
-    for args, code in [((1, 10, 0), R.ROSEN_EINVAL), ((8, 0, 0), R.ROSEN_EINVAL), ((513, 10, 0), R.ROSEN_ERANGE)]:
+    for args, code in [((1, 10, 0), R.ROSEN_EINVAL), ((8, 0, 0), R.ROSEN_EINVAL), ((16384, 10, 0), R.ROSEN_ERANGE)]:
         with pytest.raises(R.RosenError) as e:
             R.rosen_lattice_generate(*args)
         assert e.value.code == code
