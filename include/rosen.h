@@ -95,7 +95,7 @@ typedef struct rosen_outputs {
  * of free ones, lnW += ln m_s, and the ((u_s * m_s) >> 32)-th free neighbour is taken, u_s being
  * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
  * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N > ROSEN_LATTICE_SCAN_MAX_N the library keeps device
- * workspace (at most 8 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
+ * workspace (at most 12 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
  * rosen_workspace_release(); the results do not depend on which kernel ran.
  */
 ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,

@@ -38,7 +38,7 @@ struct Scratch {
     void*          hash_rec = nullptr;     size_t hash_rec_bytes = 0;
     unsigned long long* hash_ticket = nullptr;
 };
-constexpr size_t kHashTableCap = (size_t)8 << 30;   // bytes of per-chain hash tables kept resident at most
+constexpr size_t kHashTableCap = (size_t)12 << 30;  // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
 Scratch g_scratch[kMaxDevices];
 std::mutex g_mutex;
@@ -197,8 +197,8 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
         hp.key0 = (uint32_t)seed; hp.key1 = (uint32_t)(seed >> 32);
         hp.ln_shift = ln_shift; hp.out = st.dev; hp.partials = sc->dev;
         rosen::partition_chains(n_chains, &hp.chunk, &hp.n_vblocks, 256u);
-        hp.log2_entries = rosen::hash_log2_entries(N);
-        const size_t table_bytes = ((size_t)16) << hp.log2_entries;      // 16-byte entries
+        hp.entries = rosen::hash_entries(N);
+        const size_t table_bytes = (size_t)16 * hp.entries;               // 16-byte entries
         int max_threads = 0;
         if (rosen::hash_max_threads(&max_threads) < 0) return fail_cuda(cudaGetLastError(), "device query");
         uint64_t threads = (n_chains + 255) / 256 * 256;

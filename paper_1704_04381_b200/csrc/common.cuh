@@ -69,8 +69,8 @@ struct HashParams {
     uint32_t   chunk;           // chains per virtual block (multiple of 256)
     uint32_t   n_vblocks;
     ChainRecord* rec;           // [n_chains]
-    uint64_t*  tables;          // [launched threads][1 << log2_entries] 16-byte entries, zeroed before the launch
-    uint32_t   log2_entries;    // entries per chain table (power of two >= N + 1)
+    uint64_t*  tables;          // [launched threads][entries] 16-byte entries, zeroed before the launch
+    uint32_t   entries;         // entries per chain table (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
 };
 
@@ -96,7 +96,7 @@ inline void partition_chains(uint64_t n_chains, uint32_t* chunk, uint32_t* n_vbl
 int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 // lattice_hash.cu: table geometry for chain length N, resident thread capacity of the device, launch (generation
 // kernel over n_threads = multiple of 256 threads, then the per-record first reduction pass).
-uint32_t hash_log2_entries(int32_t N);
+uint32_t hash_entries(int32_t N);
 int hash_max_threads(int* threads_out);
 int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);

@@ -11,8 +11,9 @@
 //       bits 39..63  the thread's chain generation (1, 2, ...): an entry whose generation differs from the current
 //                    chain's is EMPTY, so tables are never cleared between chains (one memset per launch)
 //   .y  bit (x&3) | (y&3) << 2 | (z&3) << 4 set = site occupied
-// Tables are open-addressed (Fibonacci hash of the cube key, linear probing, no deletions) with a power of two
-// >= N+1 entries: a chain of N monomers touches at most N cubes, so a probe always ends at an empty entry.
+// Tables are open-addressed (Fibonacci hash of the cube key reduced by a multiply-high, linear probing, no deletions)
+// with N+1 entries (rounded up to even): a chain of N monomers touches at most N cubes, so a probe always ends at an
+// empty entry; on average a chain touches about N/6 cubes, so probes longer than one entry are rare.
 // The growth point's own cube lives in registers (bitmap + entry index); of the six neighbour sites only those
 // across a cube face need memory: at most three look-ups per step, 1.5 on average, against five for a per-site set,
 // and the insert is a 16-byte store to an entry that is already known.
@@ -46,9 +47,10 @@ __device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t
     return (h ^ (uint64_t)(m | (choice << 8))) * 0x100000001B3ull;
 }
 
-__device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t shift)
+// home entry of a cube: top 32 bits of the Fibonacci hash, range-reduced to [0, entries) by a multiply-high
+__device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t entries)
 {
-    return (uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> shift);
+    return __umulhi((uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> 32), entries);
 }
 
 __device__ __forceinline__ ulonglong2 load_entry(const ulonglong2* table, uint32_t slot) { return table[slot]; }
@@ -64,16 +66,16 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
     __syncthreads();
 
     const int N = p.N;
-    const uint32_t shift = 64u - p.log2_entries, mask = (1u << p.log2_entries) - 1u;
-    const uint64_t entries = 1ull << p.log2_entries;
+    const uint32_t entries = p.entries;
     ulonglong2* table = reinterpret_cast<ulonglong2*>(p.tables) + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * entries;
     uint32_t gen = 0;
+    uint32_t t = 0;                         // warp iteration counter (uniform): Philox blocks are drawn when t & 3 == 0
 
     // per-lane state of the chain being grown; s == 0: the lane needs a new chain
     uint64_t idx = 0, tag = 0, dg = 0;
     uint64_t cube = 0, bits = 0;            // the growth point's cube: key and occupancy bitmap (register copy of its entry)
     uint32_t slot = 0, l = 0;               // its entry index; local site index of the growth point inside it
-    uint32_t c_lo = 0, c_hi = 0, w[4] = {0u, 0u, 0u, 0u};
+    uint32_t c_lo = 0, c_hi = 0, w[4] = {0u, 0u, 0u, 0u}, wn[4] = {0u, 0u, 0u, 0u};
     int s = 0, x = 0, y = 0, z = 0, sx = 0, sy = 0, sz = 0;
     long long s2 = 0;
     double lnW = 0.0;
@@ -91,13 +93,13 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             const uint64_t chain = p.chain_offset + idx;
             c_lo = (uint32_t)chain; c_hi = (uint32_t)(chain >> 32);
             if (++gen > kGenMax) {     // generation counter wrapped: clear the table once and start over
-                for (uint64_t i = 0; i < entries; ++i) table[i] = make_ulonglong2(0ull, 0ull);
+                for (uint32_t i = 0; i < entries; ++i) table[i] = make_ulonglong2(0ull, 0ull);
                 gen = 1u;
             }
             tag = (uint64_t)gen << kGenShift;
             // ---- L0: r_0 = origin; every entry is empty for a new generation, so the origin's cube takes its home slot
             cube = kOriginCube; bits = 1ull; l = 0u;
-            slot = slot_of(cube, shift);
+            slot = slot_of(cube, entries);
             table[slot] = make_ulonglong2(cube | tag, bits);
             x = y = z = sx = sy = sz = 0; s2 = 0; lnW = 0.0; s = 1;
             dg = 0xCBF29CE484222325ull;
@@ -107,37 +109,45 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
                 crow = p.out.conf ? reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3 : nullptr;
                 if (crow) { crow[0] = 0; crow[1] = 0; crow[2] = 0; }
             }
-        } else if ((s & 3) == 0) {
-            philox4x32_10(c_lo, c_hi, (uint32_t)(s >> 2), 0u, p.key0, p.key1, w);   // L1
         }
+        // ---- L1. Lanes are at different steps of their chains; drawing a block whenever some lane enters a new group
+        // of four steps would run the Philox rounds in almost every iteration for a few lanes. Instead every fourth
+        // iteration ALL lanes draw the block of the next group they will enter, (s+3) >> 2 (the current group if
+        // s & 3 == 0), into wn, and a lane switches to it on entering that group -- which happens within four steps.
+        if ((t & 3u) == 0u) philox4x32_10(c_lo, c_hi, (uint32_t)(s + 3) >> 2, 0u, p.key0, p.key1, wn);
+        ++t;
+        if ((s & 3) == 0) { w[0] = wn[0]; w[1] = wn[1]; w[2] = wn[2]; w[3] = wn[3]; }
 
         // ---- L2. Per axis at most one neighbour site lies across a cube face (local coordinate 0 or 3): fetch that
         // cube's bitmap (all first probes in flight together); the other neighbours are bits of the register bitmap.
         uint64_t nkey[3], nbits[3];
         uint32_t nslot[3], nl[3];
-        bool need[3];
         ulonglong2 first[3];
+        bool need[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             const uint32_t la = (l >> (2 * a)) & 3u;
             const bool up = la == 3u;
             need[a] = up || la == 0u;
             nkey[a] = up ? cube + (1ull << (kCubeField * a)) : cube - (1ull << (kCubeField * a));
-            nl[a] = up ? l - (3u << (2 * a)) : l + (3u << (2 * a));
-            nslot[a] = slot_of(nkey[a], shift);
-            first[a] = make_ulonglong2(0ull, 0ull);
-            if (need[a]) first[a] = load_entry(table, nslot[a]);
+            nl[a] = (up ? l - (3u << (2 * a)) : l + (3u << (2 * a))) & 63u;
+            // no face on this axis: probe the growth point's own entry instead (cached, never a match for nkey, never
+            // empty) so that the load needs no branch; its result is not used
+            nslot[a] = need[a] ? slot_of(nkey[a], entries) : slot;
+            first[a] = table[nslot[a]];
         }
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            nbits[a] = 0ull;
-            if (need[a]) {
-                ulonglong2 e = first[a];
+            const uint64_t want = nkey[a] | tag;
+            const bool hit = first[a].x == want;
+            nbits[a] = hit ? first[a].y : 0ull;
+            if (need[a] && (uint32_t)(first[a].x >> kGenShift) == gen && !hit) {
+                // home entry taken by another cube of this chain (rare: tables are at most ~1/6 full on average)
                 for (;;) {
+                    nslot[a] = nslot[a] + 1u == entries ? 0u : nslot[a] + 1u;
+                    const ulonglong2 e = table[nslot[a]];
                     if ((uint32_t)(e.x >> kGenShift) != gen) break;                    // empty: cube not visited yet; nslot = where it would go
-                    if (e.x == (nkey[a] | tag)) { nbits[a] = e.y; break; }
-                    nslot[a] = (nslot[a] + 1u) & mask;
-                    e = load_entry(table, nslot[a]);
+                    if (e.x == want) { nbits[a] = e.y; break; }
                 }
             }
         }
@@ -147,7 +157,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             const uint32_t la = (l >> (2 * a)) & 3u;
             const uint32_t in_up = (uint32_t)(bits >> ((l + (1u << (2 * a))) & 63u)) & 1u;
             const uint32_t in_dn = (uint32_t)(bits >> ((l - (1u << (2 * a))) & 63u)) & 1u;
-            const uint32_t out = (uint32_t)(nbits[a] >> (nl[a] & 63u)) & 1u;
+            const uint32_t out = (uint32_t)(nbits[a] >> nl[a]) & 1u;
             occ |= (la == 3u ? out : in_up) << (2 * a);             // +axis
             occ |= (la == 0u ? out : in_dn) << (2 * a + 1);         // -axis
         }
@@ -169,14 +179,12 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             const uint32_t a = d >> 1;
             const bool up = (d & 1u) == 0u;
             const uint32_t la = (l >> (2u * a)) & 3u;
-            if (up ? la == 3u : la == 0u) {          // across a cube face: that cube's entry becomes the register copy
-                cube = pick(a, nkey[0], nkey[1], nkey[2]);
-                slot = pick(a, nslot[0], nslot[1], nslot[2]);
-                l = pick(a, nl[0], nl[1], nl[2]);
-                bits = pick(a, nbits[0], nbits[1], nbits[2]);
-            } else {
-                l = up ? l + (1u << (2u * a)) : l - (1u << (2u * a));
-            }
+            const bool cross = up ? la == 3u : la == 0u;      // across a cube face: that cube's entry becomes the register copy
+            const uint32_t l_in = up ? l + (1u << (2u * a)) : l - (1u << (2u * a));
+            cube = cross ? pick(a, nkey[0], nkey[1], nkey[2]) : cube;
+            slot = cross ? pick(a, nslot[0], nslot[1], nslot[2]) : slot;
+            bits = cross ? pick(a, nbits[0], nbits[1], nbits[2]) : bits;
+            l = cross ? pick(a, nl[0], nl[1], nl[2]) : l_in;
             bits |= 1ull << l;
             table[slot] = make_ulonglong2(cube | tag, bits);              // insert r_s (write-through; L2 absorbs repeats)
             const int sg = up ? 1 : -1;
@@ -238,11 +246,9 @@ __global__ void __launch_bounds__(256) reduce_records_kernel(const ChainRecord* 
 
 }  // namespace
 
-uint32_t hash_log2_entries(int32_t N)
+uint32_t hash_entries(int32_t N)
 {
-    uint32_t lg = 2;                                   // entries = 1 << lg >= N + 1 > cubes one chain can touch
-    while ((1ull << lg) < (uint64_t)N + 1ull) ++lg;
-    return lg;
+    return ((uint32_t)N + 2u) & ~1u;                   // even and >= N + 1 > cubes one chain can touch
 }
 
 int hash_max_threads(int* threads_out)
