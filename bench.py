@@ -47,6 +47,9 @@ def lattice_site_tests(N: int) -> int:
     return sum(max(0, s // 2 - 1) for s in range(1, N))
 
 
+HASH_INSTR_PER_STEP = 123.5     # long lattice chains (N > 512), per attempted step; see run_product
+
+
 def algorithmic_thread_instr(w: workloads.Workload) -> float:
     if w.kind == "lattice":
         # 6 equality tests per site test + one Philox block (~70 instr) per 4 steps + ~20 per step for
@@ -62,7 +65,8 @@ def algorithmic_thread_instr(w: workloads.Workload) -> float:
 def profile_traffic(w: workloads.Workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu summary of
     this workload (profiles/), per launch; None if no capture is committed."""
-    name = {"lattice_N64_2p24": "r01d_lattice_cfg2.md", "realspace_N64_k16_2p22": "r01d_realspace_cfg3.md"}.get(w.name)
+    name = {"lattice_N64_2p24": "r01d_lattice_cfg2.md", "realspace_N64_k16_2p22": "r01d_realspace_cfg3.md",
+            "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md"}.get(w.name)
     path = os.path.join(ROOT, "profiles", name) if name else None
     if not path or not os.path.exists(path):
         return None
@@ -340,21 +344,21 @@ def run_product(args, w, rank, world, local_rank):
     alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
     achieved = alg_winst / (kernel_ms * 1e-3)
     if w.kind == "lattice" and w.N > 512:
-        # hash-set kernel: per ATTEMPTED step 5 neighbour look-ups of one 32-byte sector each and one
-        # inserted key whose sector is written back = 192 algorithmic bytes, random sectors of per-chain tables in HBM
-        alg_bytes = 192.0 * steps_attempted / world
-        hbm = float(peaks.get("hbm_gbs", 6650.0))
-        roofline = {"bound": "hbm", "achieved": alg_bytes / (kernel_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
-                    "frac": alg_bytes / (kernel_ms * 1e-3) / 1e9 / hbm, "traffic": profile_traffic(w), "kernel": kernel_name,
-                    "kernel_ms": kernel_ms, "peak_source": f"hbm_gbs ({peaks_src} MEASURED_PEAKS.json; copy bandwidth, burst)",
-                    "algorithmic_bytes_per_attempted_step": 192.0,
-                    "note": "kernel_ms covers table memset + generation kernel + record reduction"}
-    else:
-      roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
+        # hash-map kernel (DESIGN.md 5.5 / 6): ncu shows it issue-bound (59.6 % issue-active, 26 % of DRAM peak), so the
+        # roofline is the issue peak; algorithmic work per ATTEMPTED step (not per nominal step: most long chains die
+        # early): 3 cube look-ups (hash 8 + compare 6 each), 6 occupancy bits (4 each), count/choose 15, insert 10,
+        # observables 12, weight 3, a quarter Philox block 17.5 = 123.5 thread-instructions
+        alg_winst = HASH_INSTR_PER_STEP * (steps_attempted / world) / 32.0
+        achieved = alg_winst / (kernel_ms * 1e-3)
+    roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
                 "frac": achieved / peak_winst, "traffic": profile_traffic(w), "kernel": kernel_name, "kernel_ms": kernel_ms,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
                 "algorithmic_thread_instr_per_chain": algorithmic_thread_instr(w)}
-    if clocks.get("sm_mhz") and roofline["bound"] == "alu":
+    if w.kind == "lattice" and w.N > 512:
+        del roofline["algorithmic_thread_instr_per_chain"]
+        roofline["algorithmic_thread_instr_per_attempted_step"] = HASH_INSTR_PER_STEP
+        roofline["note"] = "kernel_ms covers table memset + generation kernel + record reduction"
+    if clocks.get("sm_mhz"):
         roofline["frac_at_measured_clock"] = achieved / (n_sm * 4 * clocks["sm_mhz"] * 1e6)
 
     out = {
