@@ -39,7 +39,7 @@ extern "C" {
 
 #define ROSEN_OK        0
 #define ROSEN_EINVAL   (-1)  /* N < 2, n_chains == 0, k_trials outside 1..255, bond_len <= 0, sigma < 0, NaN/inf */
-#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 16383, real space 2048)           */
+#define ROSEN_ERANGE   (-2)  /* N beyond the supported chain length (lattice 16383, real space 16383)            */
 #define ROSEN_ECUDA    (-3)  /* a CUDA runtime call failed (no device, launch error, ...); see rosen_last_error */
 #define ROSEN_ENOMEM   (-4)  /* staging / workspace allocation failed                                           */
 
@@ -49,7 +49,10 @@ extern "C" {
 #define ROSEN_LATTICE_SCAN_MAX_N 512  /* up to here: chain in shared memory, parity-split scan (lattice.cu)          */
 #define ROSEN_LATTICE_MAX_N  16383   /* beyond: per-chain hash set in HBM (lattice_hash.cu), the range of the paper's
                                         "global-memory version", Table 1 PAPER.md:282-288 (N = 100 ... 10000)        */
-#define ROSEN_REALSPACE_MAX_N 2048   /* the paper's longest shared-memory chain, Table 2 */
+#define ROSEN_REALSPACE_SCAN_MAX_N 2048  /* up to here: chain in shared memory (realspace.cu); the paper's longest
+                                           shared-memory chain, Table 2                                  */
+#define ROSEN_REALSPACE_MAX_N 16383     /* beyond: chain + cell list in HBM, one warp per chain (realspace_long.cu),
+                                           the range of Table 2's "global-memory version" rows, PAPER.md:315-320      */
 
 /*
  * Ensemble summary, Eq. 2 and Eq. 6 (:362). w_c = exp(lnW_c - ln_shift) for a chain
@@ -108,7 +111,8 @@ ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed
  * fma(bond_len, u_t, r_{s-1}); it overlaps if fma(dz,dz,fma(dy,dy,dx*dx)) < sigma*sigma (fp32)
  * for some j <= s-2; m_s = number of non-overlapping trials; the ((u_s*m_s)>>32)-th of them in
  * trial order is taken, u_s as in the lattice call. 2 <= N <= ROSEN_REALSPACE_MAX_N,
- * 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, both finite.
+ * 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, both finite. N > ROSEN_REALSPACE_SCAN_MAX_N uses the library's
+ * long-chain workspace like the lattice call.
  */
 ROSEN_API int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
                              uint64_t seed, uint64_t chain_offset,

@@ -79,6 +79,14 @@ int32_t hash_min_n()
     return ROSEN_LATTICE_SCAN_MAX_N + 1;
 }
 
+// same for the real-space call (cell-list kernel, realspace_long.cu); ROSEN_REALSPACE_CELL_MIN_N overrides it
+int32_t cell_min_n()
+{
+    const char* e = std::getenv("ROSEN_REALSPACE_CELL_MIN_N");
+    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_REALSPACE_MAX_N) return (int32_t)v; }
+    return ROSEN_REALSPACE_SCAN_MAX_N + 1;
+}
+
 struct Sizes { size_t lnW, alive, m_seq, digest, conf, ree2, rg2; };
 
 Sizes output_sizes(int32_t N, uint64_t n, size_t conf_elem)
@@ -255,17 +263,58 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
     Staging st;
     if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
 
+    const float sigma2 = sigma * sigma;         // fp32 product, rounded once
+    // conservative candidate radius, rounded up: ((b + sigma)(1 + 2^-9))^2
+    const double cand_r = ((double)bond_len + (double)sigma) * (1.0 + 1.0 / 512.0);
+    float prefilter2 = (float)(cand_r * cand_r);
+    if ((double)prefilter2 < cand_r * cand_r) prefilter2 = std::nextafterf(prefilter2, INFINITY);
+    const double ln_shift = (double)(N - 1) * std::log((double)k_trials);
+
+    if (N >= cell_min_n()) {
+        // long chains: chain, cell table and cell lists in HBM, one warp per chain (realspace_long.cu)
+        rosen::RealLongParams lp{};
+        lp.N = N; lp.k = k_trials; lp.n_chains = n_chains; lp.chain_offset = chain_offset;
+        lp.key0 = (uint32_t)seed; lp.key1 = (uint32_t)(seed >> 32);
+        lp.b = bond_len; lp.sigma2 = sigma2; lp.prefilter2 = prefilter2;
+        lp.inv_cell = (float)(1.0 / (cand_r * (1.0 + 1.0 / 64.0)));
+        lp.ln_shift = ln_shift; lp.out = st.dev; lp.partials = sc->dev;
+        rosen::partition_chains(n_chains, &lp.chunk, &lp.n_vblocks, 256u);
+        lp.n_pad = ((uint32_t)N + 7u) & ~7u;
+        lp.entries = rosen::hash_entries(N);
+        lp.cand_cap = rosen::kRealLongCandCap;
+        if (const char* e = std::getenv("ROSEN_REALSPACE_CAND_CAP")) {   // test hook: force the flush path (results do not depend on it)
+            const long v = std::strtol(e, nullptr, 10);
+            if (v >= 33 && v <= (long)rosen::kRealLongCandCap) lp.cand_cap = (uint32_t)v;
+        }
+        lp.warp_bytes = ((uint64_t)lp.n_pad * 18u + (uint64_t)lp.entries * 16u + 255u) & ~(uint64_t)255u;
+        int max_warps = 0;
+        if (rosen::real_long_max_warps(k_trials, &max_warps) < 0) return fail_cuda(cudaGetLastError(), "device query");
+        uint64_t warps = (n_chains + 7) / 8 * 8;
+        if (warps > (uint64_t)max_warps) warps = (uint64_t)max_warps;
+        const uint64_t by_mem = kHashTableCap / lp.warp_bytes / 8 * 8;
+        if (warps > by_mem) warps = by_mem;
+        {
+            std::lock_guard<std::mutex> lock(g_mutex);
+            if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, warps * lp.warp_bytes))) return rc;
+            if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
+            if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
+        }
+        lp.work = static_cast<unsigned char*>(sc->hash_tables);
+        lp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
+        lp.ticket = sc->hash_ticket;
+        CK(cudaMemsetAsync(lp.work, 0, warps * lp.warp_bytes, stream));         // generation 0 = empty everywhere
+        CK(cudaMemsetAsync(lp.ticket, 0, sizeof(unsigned long long), stream));
+        rc = rosen::launch_realspace_long(lp, (int)warps, stream, &g_kernel);
+        if (rc < 0) return fail_cuda(cudaGetLastError(), "real-space long-chain kernel launch");
+        g_launches += rc;
+        return finish(sc, (int)lp.n_vblocks, n_chains, ln_shift, outputs, z, st, summary, summary_dev, stream);
+    }
+
     rosen::RealParams p{};
     p.N = N; p.k = k_trials; p.n_chains = n_chains; p.chain_offset = chain_offset;
     p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
-    p.b = bond_len; p.sigma2 = sigma * sigma;   // fp32 product, rounded once
-    {   // conservative candidate radius, rounded up: ((b + sigma)(1 + 2^-9))^2
-        const double r = ((double)bond_len + (double)sigma) * (1.0 + 1.0 / 512.0);
-        float r2 = (float)(r * r);
-        if ((double)r2 < r * r) r2 = std::nextafterf(r2, INFINITY);
-        p.prefilter2 = r2;
-    }
-    p.ln_shift = (double)(N - 1) * std::log((double)k_trials);
+    p.b = bond_len; p.sigma2 = sigma2; p.prefilter2 = prefilter2;
+    p.ln_shift = ln_shift;
     p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
     rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks, 256u);
     CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));

@@ -74,6 +74,31 @@ struct HashParams {
     unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
 };
 
+constexpr uint32_t kRealLongCandCap = 160;
+
+// Long-chain real-space path (realspace_long.cu): one warp grows one chain; chain, cell table and cell lists in HBM.
+struct RealLongParams {
+    int32_t    N;
+    int32_t    k;
+    uint64_t   n_chains;
+    uint64_t   chain_offset;
+    uint32_t   key0, key1;
+    float      b, sigma2, prefilter2;   // as RealParams
+    float      inv_cell;        // 1 / cell edge; cell edge >= candidate radius x (1 + 2^-6)
+    double     ln_shift;
+    DevOutputs out;
+    Partial*   partials;        // [n_vblocks]
+    uint32_t   chunk;           // chains per virtual block (multiple of 256)
+    uint32_t   n_vblocks;
+    ChainRecord* rec;           // [n_chains]
+    unsigned char* work;        // [launched warps][warp_bytes], zeroed before the launch
+    uint64_t   warp_bytes;      // float4 r[n_pad] | 16-byte cell entries [entries] | uint16 next[n_pad], padded to 256
+    uint32_t   n_pad;           // N rounded up to 8
+    uint32_t   cand_cap;        // candidates buffered per warp before a flush: 33 .. kRealLongCandCap
+    uint32_t   entries;         // cell-table entries per chain (even, >= N + 1)
+    unsigned long long* ticket; // zeroed before the launch: warps draw chain indices from it (load balance only)
+};
+
 // The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the
 // chain range [v*chunk, (v+1)*chunk) and produces partials[v] with a fixed thread mapping and tree, so
 // the sums depend on (n_chains, N) only -- never on the grid size, occupancy, output variant or GPU.
@@ -99,6 +124,12 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
 uint32_t hash_entries(int32_t N);
 int hash_max_threads(int* threads_out);
 int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name);
+// reduce_records_kernel of lattice_hash.cu: first reduction pass over per-chain records (+ optional per-chain outputs)
+int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks, double ln_shift,
+                          const DevOutputs& out, Partial* partials, cudaStream_t stream);
+// realspace_long.cu: resident warp capacity, launch over n_warps (multiple of 8) warps + the record reduction
+int real_long_max_warps(int k, int* warps_out);
+int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift,
                     void* summary_dev, cudaStream_t stream);   // summary_dev: rosen_summary* in device memory

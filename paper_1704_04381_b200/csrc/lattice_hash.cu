@@ -273,9 +273,15 @@ int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream,
     if (traj) { *kernel_name = "lattice_hash_kernel<traj>"; lattice_hash_kernel<true><<<grid, 256, 0, stream>>>(p); }
     else      { *kernel_name = "lattice_hash_kernel";       lattice_hash_kernel<false><<<grid, 256, 0, stream>>>(p); }
     if (cudaGetLastError() != cudaSuccess) return -3;
-    reduce_records_kernel<<<p.n_vblocks, 256, 0, stream>>>(p.rec, p.n_chains, p.chunk, p.ln_shift, p.out, p.partials);
-    if (cudaGetLastError() != cudaSuccess) return -3;
+    if (launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.out, p.partials, stream) < 0) return -3;
     return 2;
+}
+
+int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks, double ln_shift,
+                          const DevOutputs& out, Partial* partials, cudaStream_t stream)
+{
+    reduce_records_kernel<<<n_vblocks, 256, 0, stream>>>(rec, n_chains, chunk, ln_shift, out, partials);
+    return cudaGetLastError() == cudaSuccess ? 1 : -3;
 }
 
 }  // namespace rosen

@@ -78,6 +78,43 @@ def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
     check(R, N, n, k, b, sigma, seed, offset)
 
 
+# Long chains (N > ROSEN_REALSPACE_SCAN_MAX_N = 2048): the cell-list kernel of realspace_long.cu, the range of the
+# paper's real-space "global-memory version" (Table 2). Same bars as the shared-memory kernel.
+@pytest.mark.parametrize("N,n,k,b,sigma,seed,offset", [
+    (2049, 12, 8, 1.0, 0.6, 21, 0), (2500, 6, 32, 1.0, 1.0, 22, 3), (3000, 8, 2, 0.5, 0.0, 23, 0),
+    (4096, 3, 65, 1.0, 0.8, 24, 1 << 34), (5000, 4, 16, 2.0, 1.0, 25, 0), (10000, 3, 4, 1.0, 0.0, 26, 0),
+    (10000, 1, 24, 1.0, 0.4, 28, 0), (16383, 1, 16, 1.0, 0.3, 27, 0),        # chosen so that chains reach full length
+])
+def test_long_chains_cell_list_kernel(R, N, n, k, b, sigma, seed, offset):
+    check(R, N, n, k, b, sigma, seed, offset)
+    assert "realspace_long_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 3
+
+
+@pytest.mark.parametrize("cap", [None, "33"])
+def test_cell_list_kernel_on_short_chains(R, monkeypatch, cap):
+    """ROSEN_REALSPACE_CELL_MIN_N routes short chains through the cell-list kernel, where the oracle's full scan is
+    cheap enough for thousands of chains and every k variant; ROSEN_REALSPACE_CAND_CAP=33 makes the candidate buffer
+    flush after every round, the path dense configurations take."""
+    monkeypatch.setenv("ROSEN_REALSPACE_CELL_MIN_N", "2")
+    if cap:
+        monkeypatch.setenv("ROSEN_REALSPACE_CAND_CAP", cap)
+    for N, n, k, b, sigma, seed in [(2, 50, 5, 1.0, 1.0, 1), (3, 3000, 16, 1.0, 1.0, 3), (16, 2001, 7, 0.7, 1.0, 6),
+                                    (64, 4000, 16, 1.0, 1.0, 3), (40, 500, 33, 1.0, 0.0, 8), (25, 300, 65, 1.0, 0.8, 11),
+                                    (18, 200, 129, 1.0, 1.0, 12), (12, 100, 255, 1.0, 1.0, 12), (256, 300, 64, 1.0, 0.8, 13),
+                                    (300, 100, 16, 0.25, 1.0, 14), (200, 100, 8, 1.0, 0.05, 15)]:
+        check(R, N, n, k, b, sigma, seed)
+        assert "realspace_long_kernel" in R.rosen_last_kernel_name()
+    s0, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3)
+    s1, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3, outputs=ALL)
+    monkeypatch.delenv("ROSEN_REALSPACE_CELL_MIN_N")
+    s2, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3)
+    assert "realspace_kernel" in R.rosen_last_kernel_name()
+    for key in s0:
+        if not key.startswith("digest"):
+            assert s0[key] == s1[key], key
+            assert s0[key] == s2[key] or math.isclose(s0[key], s2[key], rel_tol=1e-12), key
+
+
 def test_summary_only_variant_bit_identical(R):
     N, n, k = 32, 20011, 16
     s0, _ = R.rosen_realspace_generate(N, n, k, 1.0, 1.0, 3)
@@ -104,7 +141,7 @@ def test_error_codes(R):
     bad = [((1, 10, 4, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 0, 1.0, 1.0, 0), R.ROSEN_EINVAL),
            ((8, 10, 256, 1.0, 1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, 0.0, 1.0, 0), R.ROSEN_EINVAL),
            ((8, 10, 4, 1.0, -1.0, 0), R.ROSEN_EINVAL), ((8, 10, 4, float("nan"), 1.0, 0), R.ROSEN_EINVAL),
-           ((2049, 10, 4, 1.0, 1.0, 0), R.ROSEN_ERANGE)]
+           ((16384, 10, 4, 1.0, 1.0, 0), R.ROSEN_ERANGE)]
     for args, code in bad:
         with pytest.raises(R.RosenError) as e:
             R.rosen_realspace_generate(*args)
