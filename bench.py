@@ -350,6 +350,13 @@ def run_product(args, w, rank, world, local_rank):
         # observables 12, weight 3, a quarter Philox block 17.5 = 123.5 thread-instructions
         alg_winst = HASH_INSTR_PER_STEP * (steps_attempted / world) / 32.0
         achieved = alg_winst / (kernel_ms * 1e-3)
+    long_real = w.kind == "realspace" and w.N > 2048
+    if long_real:
+        # cell-list kernel (DESIGN.md 5.6 / 6), per ATTEMPTED step: k trials x (35 Philox + 45 direction + 7 x 3.2 candidate
+        # pair tests) + 27 cell look-ups x 14 + ~40 listed monomers x 10 (candidate test) + 50 for count/choose/place/sums
+        real_long_instr = w.k_trials * (80.0 + 7.0 * 3.2) + 27 * 14.0 + 40 * 10.0 + 50.0
+        alg_winst = real_long_instr * (steps_attempted / world) / 32.0
+        achieved = alg_winst / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
                 "frac": achieved / peak_winst, "traffic": profile_traffic(w), "kernel": kernel_name, "kernel_ms": kernel_ms,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
@@ -358,6 +365,10 @@ def run_product(args, w, rank, world, local_rank):
         del roofline["algorithmic_thread_instr_per_chain"]
         roofline["algorithmic_thread_instr_per_attempted_step"] = HASH_INSTR_PER_STEP
         roofline["note"] = "kernel_ms covers table memset + generation kernel + record reduction"
+    if long_real:
+        del roofline["algorithmic_thread_instr_per_chain"]
+        roofline["algorithmic_thread_instr_per_attempted_step"] = real_long_instr
+        roofline["note"] = "kernel_ms covers workspace memset + generation kernel + record reduction"
     if clocks.get("sm_mhz"):
         roofline["frac_at_measured_clock"] = achieved / (n_sm * 4 * clocks["sm_mhz"] * 1e6)
 

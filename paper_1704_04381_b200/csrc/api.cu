@@ -286,7 +286,7 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
             const long v = std::strtol(e, nullptr, 10);
             if (v >= 33 && v <= (long)rosen::kRealLongCandCap) lp.cand_cap = (uint32_t)v;
         }
-        lp.warp_bytes = ((uint64_t)lp.n_pad * 18u + (uint64_t)lp.entries * 16u + 255u) & ~(uint64_t)255u;
+        lp.warp_bytes = ((uint64_t)lp.n_pad * 16u + (uint64_t)lp.entries * 16u + 255u) & ~(uint64_t)255u;
         int max_warps = 0;
         if (rosen::real_long_max_warps(k_trials, &max_warps) < 0) return fail_cuda(cudaGetLastError(), "device query");
         uint64_t warps = (n_chains + 7) / 8 * 8;

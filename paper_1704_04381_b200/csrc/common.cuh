@@ -92,7 +92,7 @@ struct RealLongParams {
     uint32_t   n_vblocks;
     ChainRecord* rec;           // [n_chains]
     unsigned char* work;        // [launched warps][warp_bytes], zeroed before the launch
-    uint64_t   warp_bytes;      // float4 r[n_pad] | 16-byte cell entries [entries] | uint16 next[n_pad], padded to 256
+    uint64_t   warp_bytes;      // float4 r[n_pad] (x, y, z, list link) | 16-byte cell entries [entries], padded to 256
     uint32_t   n_pad;           // N rounded up to 8
     uint32_t   cand_cap;        // candidates buffered per warp before a flush: 33 .. kRealLongCandCap
     uint32_t   entries;         // cell-table entries per chain (even, >= N + 1)

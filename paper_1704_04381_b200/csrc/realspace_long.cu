@@ -5,10 +5,10 @@
 // O(N^2): only monomers in the 27 cells around the growth point can lie inside the candidate radius.
 //
 // Layout. One warp grows one chain. Per warp, in HBM:
-//   float4   r[n_pad]            the chain (x, y, z, unused)
+//   float4   r[n_pad]            the chain: (x, y, z, link), link = bits of the index of the monomer placed before this one
+//                                in the same cell (0xFFFF: none) -- one 16-byte load per hop of a list walk
 //   entry    table[entries]      open-addressed map cell -> most recent monomer in it: 16 bytes,
 //                                .x = (cx+2^14) | (cy+2^14) << 15 | (cz+2^14) << 30 | generation << 45, .y = monomer index
-//   uint16   next[n_pad]         the monomer placed before this one in the same cell (0xFFFF: none)
 // cell = floor(coordinate * inv_cell) with cell edge = candidate radius x (1 + 2^-6): the slack covers the fp32
 // rounding of the product (|x| <= 16383 b: error < 2^-9 cells), so |x_j - x_h| < radius implies cells differ by <= 1.
 // Entries of another generation are empty (one memset per launch); entries >= N + 1 > cells a chain can touch.
@@ -81,7 +81,6 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
     unsigned char* base = p.work + ((uint64_t)blockIdx.x * kWarpsPerBlock + warp) * p.warp_bytes;
     float4* R4 = reinterpret_cast<float4*>(base);
     ulonglong2* table = reinterpret_cast<ulonglong2*>(base + (size_t)p.n_pad * 16);
-    uint16_t* next = reinterpret_cast<uint16_t*>(base + (size_t)p.n_pad * 16 + (size_t)entries * 16);
     // this lane's cell offset among the 27 (lanes 27..31 idle in the look-up)
     const int ox = lane % 3 - 1, oy = (lane / 3) % 3 - 1, oz = lane / 9 - 1;
     uint32_t gen = 0;
@@ -103,8 +102,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
         // ---- R0: r_0 = origin, alone in its cell
         float hx = 0.f, hy = 0.f, hz = 0.f;
         if (lane == 0) {
-            R4[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-            next[0] = (uint16_t)kNone;
+            R4[0] = make_float4(0.f, 0.f, 0.f, __uint_as_float(kNone));
             const uint64_t key0 = cell_key(0, 0, 0);
             table[slot_of(key0, entries)] = make_ulonglong2(key0 | tag, 0ull);
         }
@@ -159,7 +157,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
                 float4 rj = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (node != kNone) {
                     rj = R4[node];
-                    const uint32_t nx = next[node];
+                    const uint32_t nx = __float_as_uint(rj.w);
                     const float ax = rj.x - hx, ay = rj.y - hy, az = rj.z - hz;
                     in = (int)node < s - 1 && fmaf(az, az, fmaf(ay, ay, ax * ax)) < p.prefilter2;
                     node = nx;
@@ -215,7 +213,6 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
 
             // store r_s and push it on its cell's list (lane 0; the warp sees it after the __syncwarp)
             if (lane == 0) {
-                R4[s] = make_float4(hx, hy, hz, 0.f);
                 const uint64_t want = cell_key(__float2int_rd(__fmul_rn(hx, p.inv_cell)), __float2int_rd(__fmul_rn(hy, p.inv_cell)),
                                                __float2int_rd(__fmul_rn(hz, p.inv_cell))) | tag;
                 uint32_t sl = slot_of(want & ~(~0ull << kGenShift), entries);
@@ -226,7 +223,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
                     if (e.x == want) { prev = (uint32_t)e.y; break; }
                     sl = sl + 1u == entries ? 0u : sl + 1u;
                 }
-                next[s] = (uint16_t)prev;
+                R4[s] = make_float4(hx, hy, hz, __uint_as_float(prev));
                 table[sl] = make_ulonglong2(want, (uint64_t)s);
             }
 
