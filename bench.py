@@ -187,7 +187,7 @@ def oracle_call(w: workloads.Workload, n_chains: int, offset: int = 0):
 
 def time_oracle(w: workloads.Workload, target_s: float):
     """Single-thread oracle on a chain-id prefix sized for about target_s seconds."""
-    probe = 64
+    probe = 64 if w.N <= 2048 else 1                     # a long chain can cost seconds by itself
     while True:
         t0 = time.perf_counter(); oracle_call(w, probe); dt = time.perf_counter() - t0
         if dt > 0.2 or probe >= w.n_chains:
@@ -215,7 +215,7 @@ def run_reference(args, w, rank):
     warmup, steps = max(args.warmup, 1), args.steps
     m0, dt0, _ = time_oracle(w, 1.0)
     budget = 120.0 / (steps + warmup)                    # whole run within a few minutes
-    m = int(max(16, min(w.n_chains, m0 / dt0 * min(budget, 2.0))))
+    m = int(max(16 if w.N <= 2048 else 1, min(w.n_chains, m0 / dt0 * min(budget, 2.0))))
     for _ in range(warmup):
         oracle_call(w, m)
     t0 = time.perf_counter()
@@ -397,7 +397,7 @@ def run_product(args, w, rank, world, local_rank):
     if world == 1 and not args.no_cpu_baseline:
         m, dt, _ = time_oracle(w, args.cpu_seconds / 2)
         cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
-        per = max(16, int(m / dt * args.cpu_seconds / 2))           # ~cpu_seconds/2 of work per thread
+        per = max(16 if w.N <= 2048 else 1, int(m / dt * args.cpu_seconds / 2))   # ~cpu_seconds/2 of work per thread
         ma, dta = time_oracle_all_cores(w, per, cores)
         out["cpu_baseline"] = {"value": ma / dta, "unit": "chains/s", "cores": cores, "kind": "oracle",
                                "sample": f"{cores} threads x {per} chains (disjoint chain-id ranges of {w.name}), {dta:.1f} s",

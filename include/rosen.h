@@ -64,8 +64,9 @@ typedef struct rosen_summary {
     uint64_t n_chains;            /* chains attempted                                                  */
     uint64_t n_dead;              /* chains that hit m_s = 0                                           */
     uint64_t n_steps_attempted;   /* sum over chains of growth steps attempted (= monomer-steps)       */
-    double   ln_shift;            /* L: lattice ln6 + (N-2) ln5 (N <= 512) or ln6 + (N-2) ln 4.684     */
-                                  /*    (N > 512, reading A16); real space (N-1) ln k        */
+    double   ln_shift;            /* L: lattice ln6 + (N-2) ln5, real space (N-1) ln k; long chains    */
+                                  /*    (lattice N > 512, real space N > 2048): the largest lnW of the */
+                                  /*    call, 0 if no chain is alive (reading A18)        */
     double   sum_w, sum_w_ree2, sum_w_rg2, sum_w2;
     double   mean_ree2;           /* sum_w_ree2 / sum_w   : W-weighted <R_ee^2>                        */
     double   mean_rg2;            /* sum_w_rg2 / sum_w    : W-weighted <R_g^2>                         */
@@ -144,7 +145,8 @@ ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trial
 /*
  * Merge the summaries of disjoint chain ranges generated with the same (N, k_trials) -- the only
  * "exchange" a multi-GPU run needs. Sums are added in array order (deterministic),
- * derived fields recomputed. Returns ROSEN_EINVAL if count == 0 or the ln_shift values differ.
+ * derived fields recomputed. Parts with different ln_shift (long chains) are rescaled to the largest shift of a
+ * part with sum_w > 0. Returns ROSEN_EINVAL if count == 0 or a shift is not finite.
  * Pure host function.
  */
 ROSEN_API int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged);

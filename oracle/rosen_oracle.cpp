@@ -144,19 +144,42 @@ static void finish_summary(oracle_summary* S, uint64_t n_chains, uint64_t n_dead
     S->digest_xor = dx; S->digest_sum = ds;
 }
 
+// Ensemble sums, Eq. 2 and Eq. 6 (:362), over the stored per-chain results in chain order.
+// `long_chain` (lattice N > 512, real space N > 2048, reading A18): the shift is the largest lnW of the
+// run instead of the fixed bound L_fixed, because exp(lnW - L_fixed) underflows fp64 for chains of 10^4 monomers.
+// Any L cancels in the ratios of Eq. 2 and is added back in Eq. 6; with no chain alive L = 0 and the means are 0/0.
+struct ChainResult { double lnW, ree2, rg2; bool alive; };
+
+static void ensemble(oracle_summary* S, const std::vector<ChainResult>& res, bool long_chain, double L_fixed,
+                     uint64_t n_steps, uint64_t dx, uint64_t ds)
+{
+    double L = L_fixed;
+    if (long_chain) {
+        bool any = false;
+        for (const ChainResult& c : res) if (c.alive && (!any || c.lnW > L)) { L = c.lnW; any = true; }
+        if (!any) L = 0.0;
+    }
+    Comp sw, swr, swg, sw2;
+    uint64_t n_dead = 0;
+    for (const ChainResult& c : res) {
+        const double w = c.alive ? std::exp(c.lnW - L) : 0.0;
+        sw.add(w); swr.add(w * c.ree2); swg.add(w * c.rg2); sw2.add(w * w);
+        if (!c.alive) ++n_dead;
+    }
+    finish_summary(S, (uint64_t)res.size(), n_dead, n_steps, L, sw, swr, swg, sw2, dx, ds);
+}
+
 // Cubic-lattice Rosenbluth generation, PAPER.md:100-179 (Alg. 1), Eq. 3 (:58), sec. 3.3.2.
 // Returns 0, or -1 on invalid arguments.
 int oracle_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
                             const oracle_outputs* out, oracle_summary* summary)
 {
     if (N < 2 || n_chains == 0) return -1;
-    // L: the largest possible lnW for N <= 512; beyond that exp(lnW - L) would underflow fp64 (lnW - L ~ -0.065 N),
-    // so long chains are shifted by the paper's growth constant mu = 4.684 (Table 4) instead
-    // (reading A16). L is a constant of N: it cancels in every ratio of Eq. 2 and is added back in Eq. 6.
-    const double L = std::log(6.0) + (double)(N - 2) * std::log(N <= 512 ? 5.0 : 4.684);
+    const double L = std::log(6.0) + (double)(N - 2) * std::log(5.0);     // max possible lnW (fixed shift, N <= 512)
     std::vector<int32_t> r((size_t)N * 3);
-    Comp sw, swr, swg, sw2;
-    uint64_t n_dead = 0, n_steps = 0, dxor = 0, dsum = 0;
+    std::vector<ChainResult> res;
+    res.reserve(n_chains);
+    uint64_t n_steps = 0, dxor = 0, dsum = 0;
 
     for (uint64_t i = 0; i < n_chains; ++i) {
         const uint64_t chain = chain_offset + i;
@@ -199,10 +222,9 @@ int oracle_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_
             ree2 = (double)(ex*ex + ey*ey + ez*ez);
             rg2  = (double)((int64_t)N * s2 - (sx*sx + sy*sy + sz*sz)) / ((double)N * (double)N);
         } else {
-            lnW = -std::numeric_limits<double>::infinity(); ++n_dead;
+            lnW = -std::numeric_limits<double>::infinity();
         }
-        const double w = alive ? std::exp(lnW - L) : 0.0;
-        sw.add(w); swr.add(w * ree2); swg.add(w * rg2); sw2.add(w * w);
+        res.push_back(ChainResult{lnW, ree2, rg2, alive});
         dxor ^= h; dsum += h;
 
         if (out) {
@@ -214,7 +236,7 @@ int oracle_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_
             if (out->conf) std::memcpy((int32_t*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(int32_t));
         }
     }
-    finish_summary(summary, n_chains, n_dead, n_steps, L, sw, swr, swg, sw2, dxor, dsum);
+    ensemble(summary, res, N > 512, L, n_steps, dxor, dsum);
     return 0;
 }
 
@@ -281,8 +303,9 @@ int oracle_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, fl
     std::vector<float> r((size_t)N * 3);
     std::vector<float> trial((size_t)k * 3);
     std::vector<int32_t> free_t((size_t)k);
-    Comp sw, swr, swg, sw2;
-    uint64_t n_dead = 0, n_steps = 0, dxor = 0, dsum = 0;
+    std::vector<ChainResult> res;
+    res.reserve(n_chains);
+    uint64_t n_steps = 0, dxor = 0, dsum = 0;
 
     for (uint64_t i = 0; i < n_chains; ++i) {
         const uint64_t chain = chain_offset + i;
@@ -342,10 +365,9 @@ int oracle_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, fl
                          ez = (double)r[3*(N-1)+2] - (double)r[2];
             ree2 = ex*ex + ey*ey + ez*ez;
         } else {
-            lnW = -std::numeric_limits<double>::infinity(); ++n_dead;
+            lnW = -std::numeric_limits<double>::infinity();
         }
-        const double w = alive ? std::exp(lnW - L) : 0.0;
-        sw.add(w); swr.add(w * ree2); swg.add(w * rg2); sw2.add(w * w);
+        res.push_back(ChainResult{lnW, ree2, rg2, alive});
         dxor ^= h; dsum += h;
 
         if (out) {
@@ -357,7 +379,7 @@ int oracle_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, fl
             if (out->conf) std::memcpy((float*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(float));
         }
     }
-    finish_summary(summary, n_chains, n_dead, n_steps, L, sw, swr, swg, sw2, dxor, dsum);
+    ensemble(summary, res, N > 2048, L, n_steps, dxor, dsum);
     return 0;
 }
 

@@ -32,6 +32,7 @@ struct Scratch {
     Partial*       dev = nullptr;          // [kMaxPartials] block partials
     rosen_summary* summary_dev = nullptr;  // written by finalize_kernel
     uint32_t*      vb_counter = nullptr;   // virtual-block ticket of the lattice kernel
+    double*        lmax = nullptr;         // [kMaxPartials + 1] block maxima of lnW and their maximum (long chains)
     rosen_summary* summary_host = nullptr; // pinned mirror
     // long-chain lattice path (lattice_hash.cu): grown on demand, kept until rosen_workspace_release()
     void*          hash_tables = nullptr;  size_t hash_tables_bytes = 0;
@@ -54,6 +55,7 @@ int get_scratch(Scratch** out)
         CK(cudaMalloc(&s.dev, sizeof(Partial) * rosen::kMaxPartials));
         CK(cudaMalloc(&s.summary_dev, sizeof(rosen_summary)));
         CK(cudaMalloc(&s.vb_counter, sizeof(uint32_t)));
+        CK(cudaMalloc(&s.lmax, sizeof(double) * (rosen::kMaxPartials + 1)));
         CK(cudaMallocHost(&s.summary_host, sizeof(rosen_summary)));
     }
     *out = &s;
@@ -163,12 +165,12 @@ void derive(rosen_summary* s)
 
 // After the generation kernel: second reduction pass, summary copy, host staging copies, sync.
 // summary (host) and summary_dev (device) are both optional; the finalize kernel runs if either is set.
-int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const rosen_outputs* outputs, const Sizes& z,
+int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const double* ln_shift_dev, const rosen_outputs* outputs, const Sizes& z,
            Staging& st, rosen_summary* summary, rosen_summary* summary_dev, cudaStream_t stream)
 {
     if (summary || summary_dev) {
         rosen_summary* target = summary_dev ? summary_dev : sc->summary_dev;
-        if (rosen::launch_finalize(sc->dev, grid, n_chains, ln_shift, target, stream) < 0)
+        if (rosen::launch_finalize(sc->dev, grid, n_chains, ln_shift, ln_shift_dev, target, stream) < 0)
             return fail_cuda(cudaGetLastError(), "finalize_kernel");
         ++g_launches;
         if (summary) CK(cudaMemcpyAsync(sc->summary_host, target, sizeof(rosen_summary), cudaMemcpyDeviceToHost, stream));
@@ -222,12 +224,13 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
         hp.tables = static_cast<uint64_t*>(sc->hash_tables);
         hp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
         hp.ticket = sc->hash_ticket;
+        hp.lmax = N > ROSEN_LATTICE_SCAN_MAX_N ? sc->lmax : nullptr;     // short chains routed here by the env override keep the fixed shift
         CK(cudaMemsetAsync(hp.tables, 0, threads * table_bytes, stream));      // generation 0 = empty everywhere
         CK(cudaMemsetAsync(hp.ticket, 0, sizeof(unsigned long long), stream));
         rc = rosen::launch_lattice_hash(hp, (int)threads, stream, &g_kernel);
         if (rc < 0) return fail_cuda(cudaGetLastError(), "lattice hash kernel launch");
         g_launches += rc;
-        return finish(sc, (int)hp.n_vblocks, n_chains, ln_shift, outputs, z, st, summary, summary_dev, stream);
+        return finish(sc, (int)hp.n_vblocks, n_chains, ln_shift, hp.lmax ? hp.lmax + rosen::kMaxPartials : nullptr, outputs, z, st, summary, summary_dev, stream);
     }
 
     rosen::LatticeParams p{};
@@ -241,7 +244,7 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");
     g_launches += rc;
-    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
+    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, outputs, z, st, summary, summary_dev, stream);
 }
 
 int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma, uint64_t seed,
@@ -302,12 +305,13 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
         lp.work = static_cast<unsigned char*>(sc->hash_tables);
         lp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
         lp.ticket = sc->hash_ticket;
+        lp.lmax = N > ROSEN_REALSPACE_SCAN_MAX_N ? sc->lmax : nullptr;   // as in the lattice call
         CK(cudaMemsetAsync(lp.work, 0, warps * lp.warp_bytes, stream));         // generation 0 = empty everywhere
         CK(cudaMemsetAsync(lp.ticket, 0, sizeof(unsigned long long), stream));
         rc = rosen::launch_realspace_long(lp, (int)warps, stream, &g_kernel);
         if (rc < 0) return fail_cuda(cudaGetLastError(), "real-space long-chain kernel launch");
         g_launches += rc;
-        return finish(sc, (int)lp.n_vblocks, n_chains, ln_shift, outputs, z, st, summary, summary_dev, stream);
+        return finish(sc, (int)lp.n_vblocks, n_chains, ln_shift, lp.lmax ? lp.lmax + rosen::kMaxPartials : nullptr, outputs, z, st, summary, summary_dev, stream);
     }
 
     rosen::RealParams p{};
@@ -322,7 +326,7 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
     rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space kernel launch");
     g_launches += rc;
-    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, outputs, z, st, summary, summary_dev, stream);
+    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, outputs, z, st, summary, summary_dev, stream);
 }
 
 }  // namespace
@@ -381,12 +385,21 @@ int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trials, float b
 int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged)
 {
     if (!parts || !merged || count < 1) return ROSEN_EINVAL;
-    rosen_summary m = parts[0];
-    for (int32_t i = 1; i < count; ++i) {
+    // common shift = the largest of the parts' (equal for short chains; per-call maxima for long chains, reading A18):
+    // sums are rescaled by exp(L_i - L) (squared for sum_w2), a factor of exactly 1 when the shifts agree
+    for (int32_t i = 0; i < count; ++i)
+        if (!std::isfinite(parts[i].ln_shift)) return ROSEN_EINVAL;
+    double L = parts[0].ln_shift;
+    bool have = parts[0].sum_w > 0.0;
+    for (int32_t i = 1; i < count; ++i)
+        if (parts[i].sum_w > 0.0 && (!have || parts[i].ln_shift > L)) { L = parts[i].ln_shift; have = true; }
+    rosen_summary m{};
+    m.ln_shift = L;
+    for (int32_t i = 0; i < count; ++i) {
         const rosen_summary& q = parts[i];
-        if (q.ln_shift != m.ln_shift) return ROSEN_EINVAL;
+        const double f = q.sum_w > 0.0 ? std::exp(q.ln_shift - L) : 0.0;
         m.n_chains += q.n_chains; m.n_dead += q.n_dead; m.n_steps_attempted += q.n_steps_attempted;
-        m.sum_w += q.sum_w; m.sum_w_ree2 += q.sum_w_ree2; m.sum_w_rg2 += q.sum_w_rg2; m.sum_w2 += q.sum_w2;
+        m.sum_w += f * q.sum_w; m.sum_w_ree2 += f * q.sum_w_ree2; m.sum_w_rg2 += f * q.sum_w_rg2; m.sum_w2 += f * f * q.sum_w2;
         m.digest_xor ^= q.digest_xor; m.digest_sum += q.digest_sum;
     }
     derive(&m);

@@ -72,6 +72,7 @@ struct HashParams {
     uint64_t*  tables;          // [launched threads][entries] 16-byte entries, zeroed before the launch
     uint32_t   entries;         // entries per chain table (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
+    double*    lmax;            // [kMaxPartials + 1] scratch, or null: N <= 512, fixed shift ln_shift (reading A18)
 };
 
 constexpr uint32_t kRealLongCandCap = 160;
@@ -97,6 +98,7 @@ struct RealLongParams {
     uint32_t   cand_cap;        // candidates buffered per warp before a flush: 33 .. kRealLongCandCap
     uint32_t   entries;         // cell-table entries per chain (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: warps draw chain indices from it (load balance only)
+    double*    lmax;            // [kMaxPartials + 1] scratch, or null: N <= 2048, fixed shift ln_shift (reading A18)
 };
 
 // The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the
@@ -125,13 +127,14 @@ uint32_t hash_entries(int32_t N);
 int hash_max_threads(int* threads_out);
 int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name);
 // reduce_records_kernel of lattice_hash.cu: first reduction pass over per-chain records (+ optional per-chain outputs)
+// lmax != nullptr: first find L = max lnW (two launches), left in lmax[kMaxPartials]. Returns the launches made.
 int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks, double ln_shift,
-                          const DevOutputs& out, Partial* partials, cudaStream_t stream);
+                          double* lmax, const DevOutputs& out, Partial* partials, cudaStream_t stream);
 // realspace_long.cu: resident warp capacity, launch over n_warps (multiple of 8) warps + the record reduction
 int real_long_max_warps(int k, int* warps_out);
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
-int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift,
+int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift, const double* ln_shift_dev,
                     void* summary_dev, cudaStream_t stream);   // summary_dev: rosen_summary* in device memory
 
 }  // namespace rosen

@@ -219,13 +219,51 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
     }
 }
 
+// Long chains proper (lattice N > 512, real space N > 2048, reading A18): the shift L of the weights is the
+// largest lnW of the call, found by two max passes over the records (max is exact and order independent) and kept
+// in device memory for the sums and for the summary. lmax[0..n_vblocks) = block maxima, lmax[kMaxPartials] = L.
+__global__ void __launch_bounds__(256) records_max_kernel(const ChainRecord* __restrict__ rec, uint64_t n_chains, uint32_t chunk,
+                                                          double* lmax)
+{
+    __shared__ double sm[8];
+    double v = -CUDART_INF;
+    for (uint32_t it = 0; it < chunk / 256u; ++it) {
+        const uint64_t idx = (uint64_t)blockIdx.x * chunk + (uint64_t)it * 256u + threadIdx.x;
+        if (idx >= n_chains) break;
+        if (rec[idx].alive != 0u) v = fmax(v, rec[idx].lnW);
+    }
+    for (int d = 16; d >= 1; d >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, d));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) v = fmax(v, sm[w]);
+        lmax[blockIdx.x] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) records_max_final_kernel(double* lmax, uint32_t n_vblocks)
+{
+    __shared__ double sm[8];
+    double v = -CUDART_INF;
+    for (uint32_t i = threadIdx.x; i < n_vblocks; i += 256u) v = fmax(v, lmax[i]);
+    for (int d = 16; d >= 1; d >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, d));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) v = fmax(v, sm[w]);
+        lmax[kMaxPartials] = v == -CUDART_INF ? 0.0 : v;       // no chain alive: L = 0, all weights 0
+    }
+}
+
 // E1, first pass, for kernels that write per-chain records: virtual block v sums the chains [v*chunk, (v+1)*chunk)
 // with the thread mapping and tree of the generation kernels (thread t takes v*chunk + it*256 + t, it ascending).
+// ln_shift_dev != nullptr: the shift is read from device memory (long chains), else ln_shift is used.
 __global__ void __launch_bounds__(256) reduce_records_kernel(const ChainRecord* __restrict__ rec, uint64_t n_chains, uint32_t chunk,
-                                                             double ln_shift, DevOutputs out, Partial* partials)
+                                                             double ln_shift, const double* ln_shift_dev, DevOutputs out, Partial* partials)
 {
     __shared__ Partial scratch[8];
     const uint32_t vb = blockIdx.x;
+    if (ln_shift_dev) ln_shift = *ln_shift_dev;
     Partial acc = partial_zero();
     for (uint32_t it = 0; it < chunk / 256u; ++it) {
         const uint64_t idx = (uint64_t)vb * chunk + (uint64_t)it * 256u + threadIdx.x;
@@ -273,15 +311,21 @@ int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream,
     if (traj) { *kernel_name = "lattice_hash_kernel<traj>"; lattice_hash_kernel<true><<<grid, 256, 0, stream>>>(p); }
     else      { *kernel_name = "lattice_hash_kernel";       lattice_hash_kernel<false><<<grid, 256, 0, stream>>>(p); }
     if (cudaGetLastError() != cudaSuccess) return -3;
-    if (launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.out, p.partials, stream) < 0) return -3;
-    return 2;
+    const int rc = launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.lmax, p.out, p.partials, stream);
+    return rc < 0 ? rc : 1 + rc;
 }
 
 int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks, double ln_shift,
-                          const DevOutputs& out, Partial* partials, cudaStream_t stream)
+                          double* lmax, const DevOutputs& out, Partial* partials, cudaStream_t stream)
 {
-    reduce_records_kernel<<<n_vblocks, 256, 0, stream>>>(rec, n_chains, chunk, ln_shift, out, partials);
-    return cudaGetLastError() == cudaSuccess ? 1 : -3;
+    int launches = 1;
+    if (lmax) {
+        records_max_kernel<<<n_vblocks, 256, 0, stream>>>(rec, n_chains, chunk, lmax);
+        records_max_final_kernel<<<1, 256, 0, stream>>>(lmax, n_vblocks);
+        launches = 3;
+    }
+    reduce_records_kernel<<<n_vblocks, 256, 0, stream>>>(rec, n_chains, chunk, ln_shift, lmax ? lmax + kMaxPartials : nullptr, out, partials);
+    return cudaGetLastError() == cudaSuccess ? launches : -3;
 }
 
 }  // namespace rosen

@@ -304,8 +304,8 @@ int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t str
     else if (p.k <= 128) { *kernel_name = "realspace_long_kernel<P=2>"; rc = launch_p<2>(p, n_warps, stream); }
     else                 { *kernel_name = "realspace_long_kernel<P=4>"; rc = launch_p<4>(p, n_warps, stream); }
     if (rc < 0) return rc;
-    if (launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.out, p.partials, stream) < 0) return -3;
-    return 2;
+    rc = launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.lmax, p.out, p.partials, stream);
+    return rc < 0 ? rc : 1 + rc;
 }
 
 }  // namespace rosen

@@ -7,8 +7,10 @@
 namespace rosen {
 
 __global__ void __launch_bounds__(256) finalize_kernel(const Partial* __restrict__ partials, int n,
-                                                       uint64_t n_chains, double ln_shift, rosen_summary* out)
+                                                       uint64_t n_chains, double ln_shift, const double* ln_shift_dev,
+                                                       rosen_summary* out)
 {
+    if (ln_shift_dev) ln_shift = *ln_shift_dev;        // long chains: L = max lnW, found on the device (reading A18)
     __shared__ Partial scratch[8];
     __shared__ Partial total;
     Partial acc = partial_zero();
@@ -28,10 +30,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(const Partial* __restrict
     }
 }
 
-int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift,
+int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift, const double* ln_shift_dev,
                     void* summary_dev, cudaStream_t stream)
 {
-    finalize_kernel<<<1, 256, 0, stream>>>(partials, n_partials, n_chains, ln_shift,
+    finalize_kernel<<<1, 256, 0, stream>>>(partials, n_partials, n_chains, ln_shift, ln_shift_dev,
                                            static_cast<rosen_summary*>(summary_dev));
     return cudaGetLastError() == cudaSuccess ? 1 : -3;
 }

@@ -1,6 +1,7 @@
 """CPU checks of the boundary: librosen.so loads, exports every symbol include/rosen.h declares, the
 pure-host entry points work, and the generate calls fail loudly (no CPU fallback) without a device."""
 import ctypes
+import math
 import os
 import re
 
@@ -50,8 +51,14 @@ def test_host_only_entry_points(R):
     m = R.rosen_summary_merge([a, b])
     assert m["n_chains"] == 40 and m["n_dead"] == 1 and m["sum_w"] == 16.0 and m["mean_ree2"] == 20.0 / 16.0
     assert m["digest_xor"] == 3 and m["digest_sum"] == 4 and m["attrition"] == 1 / 40
+    # different shifts (long chains, reading A18): rescaled to the largest, exp(2 - 3) on the sums of the first part
+    m = R.rosen_summary_merge([a, dict(b, ln_shift=3.0)])
+    f = math.exp(-1.0)
+    assert m["ln_shift"] == 3.0 and math.isclose(m["sum_w"], 4.0 * f + 12.0, rel_tol=1e-15)
+    assert math.isclose(m["sum_w2"], 3.0 * f * f + 3.0, rel_tol=1e-15)
+    assert math.isclose(m["ln_mean_W"], 3.0 + math.log((4.0 * f + 12.0) / 40), rel_tol=1e-15)
     with pytest.raises(R.RosenError):
-        R.rosen_summary_merge([a, dict(b, ln_shift=3.0)])
+        R.rosen_summary_merge([a, dict(b, ln_shift=float("inf"))])
 
 
 def test_no_cpu_fallback(R):

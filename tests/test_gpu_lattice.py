@@ -79,7 +79,7 @@ def test_shapes_ragged_and_edges(R, N, n_chains, seed, offset):
 ])
 def test_long_chains_hash_kernel(R, N, n_chains, seed, offset):
     s, t = R.rosen_lattice_generate(N, n_chains, seed, chain_offset=offset, outputs=ALL)
-    assert "lattice_hash_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 3
+    assert "lattice_hash_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 5
     o = oracle.lattice_generate(N, n_chains, seed, chain_offset=offset)
     compare_per_chain(t, o, N)
     compare_summary(s, o.summary)
@@ -126,7 +126,7 @@ def test_long_chain_properties_at_bench_size(R):
     assert s["n_dead"] == int((~alive).sum()) and 0.1 < s["attrition"] < 0.35
     assert bool(torch.isinf(t["lnW"][~alive]).all()) and bool((t["ree2"][~alive] == 0).all())
     L = s["ln_shift"]
-    assert bool((t["lnW"][alive] <= math.log(6.0) + (N - 2) * math.log(5.0) + 1e-9).all()) and abs(L - (math.log(6.0) + (N - 2) * math.log(4.684))) < 1e-9 and bool((t["ree2"][alive] <= (N - 1) ** 2).all())
+    assert bool((t["lnW"][alive] <= math.log(6.0) + (N - 2) * math.log(5.0) + 1e-9).all()) and L == float(t["lnW"][alive].max()) and bool((t["ree2"][alive] <= (N - 1) ** 2).all())
     assert bool((t["ree2"][alive] % 2 == (N - 1) % 2).all())           # bipartite lattice: parity of |r|^2 = parity of the step count
     for off in (0, 77777, n - 3):
         o = oracle.lattice_generate(N, 3, seed, chain_offset=off)

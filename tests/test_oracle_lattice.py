@@ -222,18 +222,26 @@ def test_invalid_arguments():
 
 
 def test_long_chain_shift_cancels_and_is_added_back():
-    """Reading A18: for N > 512 the oracle normalises with L = ln6 + (N-2) ln 4.684 (mu of Table 4,
-    PAPER.md:373). L must cancel in Eq. 2 and be added back in Eq. 6: the summary equals a log-sum-exp computed here
-    from the per-chain lnW with NO shift constant at all, and the N = 512 / 513 pair brackets the switch."""
-    for N, base in ((512, 5.0), (513, 4.684), (1500, 4.684)):
-        r = oracle.lattice_generate(N, 300, 31)
+    """Reading A18: for N > 512 the oracle normalises with L = the largest lnW of the run (the fixed
+    bound ln6 + (N-2) ln5 underflows fp64 at N ~ 10^4). L must cancel in Eq. 2 and be added back in Eq. 6: the summary
+    equals a log-sum-exp computed here from the per-chain lnW, and the N = 512 / 513 pair brackets the switch."""
+    for N in (512, 513, 1500, 6000):
+        r = oracle.lattice_generate(N, 300 if N < 6000 else 60, 31)
         S = r.summary
-        assert math.isclose(S["ln_shift"], math.log(6.0) + (N - 2) * math.log(base), rel_tol=1e-15)
         a = r.alive == 1
         lnw = r.lnW[a]
         top = lnw.max()
-        rel = np.exp(lnw - top)                                     # shift-free: own maximum
+        if N <= 512:
+            assert math.isclose(S["ln_shift"], math.log(6.0) + (N - 2) * math.log(5.0), rel_tol=1e-15)
+        else:
+            assert S["ln_shift"] == top
+            assert S["sum_w"] >= 1.0 and S["sum_w2"] >= 1.0            # the heaviest chain has w = 1 exactly
+        rel = np.exp(lnw - top)
         assert math.isclose(S["ln_mean_W"], top + math.log(rel.sum() / r.alive.size), rel_tol=1e-12)
         assert math.isclose(S["mean_ree2"], float((rel * r.ree2[a]).sum() / rel.sum()), rel_tol=1e-12)
         assert math.isclose(S["mean_rg2"], float((rel * r.rg2[a]).sum() / rel.sum()), rel_tol=1e-12)
         assert S["n_dead"] == int((~a).sum()) and 0 < S["sum_w"] < float("inf") and S["sum_w2"] > 0
+    # no chain alive: L = 0, sums 0, means 0/0
+    r = oracle.lattice_generate(16383, 3, 20)
+    assert r.summary["n_dead"] == 3 and r.summary["ln_shift"] == 0.0 and r.summary["sum_w"] == 0.0
+    assert math.isnan(r.summary["mean_ree2"])

@@ -190,3 +190,21 @@ def test_scaling_exponent_consistency_P10():
     nu_rs = np.polyfit(x, np.log(rs), 1)[0] / 2
     assert 0.56 < nu_lat < 0.64 and 0.56 < nu_rs < 0.66
     assert abs(nu_lat - nu_rs) < 0.05
+
+
+def test_long_chain_shift_is_the_largest_lnW():
+    """Reading A18 for real space (N > 2048): L = max lnW instead of (N-1) ln k, which underflows exp(lnW - L) for
+    chains of 10^4 monomers (lnW - (N-1) ln k ~ N ln(free fraction)). Checked against a shift-free log-sum-exp."""
+    for N, k, sigma in ((2048, 4, 0.3), (2049, 4, 0.3)):
+        r = oracle.realspace_generate(N, 6, k, 1.0, sigma, 5)
+        S = r.summary
+        a = r.alive == 1
+        assert a.any()
+        top = r.lnW[a].max()
+        if N <= 2048:
+            assert math.isclose(S["ln_shift"], (N - 1) * math.log(k), rel_tol=1e-15)
+        else:
+            assert S["ln_shift"] == top and S["sum_w"] >= 1.0
+        rel = np.exp(r.lnW[a] - top)
+        assert math.isclose(S["ln_mean_W"], top + math.log(rel.sum() / a.size), rel_tol=1e-12)
+        assert math.isclose(S["mean_ree2"], float((rel * r.ree2[a]).sum() / rel.sum()), rel_tol=1e-12)
