@@ -46,7 +46,8 @@ extern "C" {
 #define ROSEN_MEM_DEVICE 0
 #define ROSEN_MEM_HOST   1
 
-#define ROSEN_LATTICE_SCAN_MAX_N 512  /* up to here: chain in shared memory, parity-split scan (lattice.cu)          */
+#define ROSEN_LATTICE_SCAN_MAX_N 512  /* longest chain of the shared-memory scan kernel (lattice.cu)                   */
+#define ROSEN_LATTICE_HASH_MIN_N 193  /* from here on the hash-map kernel is faster and is used (measured crossover)   */
 #define ROSEN_LATTICE_MAX_N  16383   /* beyond: per-chain hash set in HBM (lattice_hash.cu), the range of the paper's
                                         "global-memory version", Table 1 PAPER.md:282-288 (N = 100 ... 10000)        */
 #define ROSEN_REALSPACE_SCAN_MAX_N 2048  /* up to here: chain in shared memory (realspace.cu); the paper's longest
@@ -98,7 +99,7 @@ typedef struct rosen_outputs {
  * r_{s-1}, in the order +x,-x,+y,-y,+z,-z, are tested against all earlier monomers, m_s = number
  * of free ones, lnW += ln m_s, and the ((u_s * m_s) >> 32)-th free neighbour is taken, u_s being
  * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
- * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N > ROSEN_LATTICE_SCAN_MAX_N the library keeps device
+ * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N >= ROSEN_LATTICE_HASH_MIN_N the library keeps device
  * workspace (at most 12 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
  * rosen_workspace_release(); the results do not depend on which kernel ran.
  */

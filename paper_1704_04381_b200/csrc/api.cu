@@ -72,13 +72,14 @@ int grow(void** ptr, size_t* have, size_t need)
     return ROSEN_OK;
 }
 
-// chain length from which the lattice call uses the hash-set kernel; ROSEN_LATTICE_HASH_MIN_N overrides it
-// (tests run the hash kernel on short chains too, where the enumeration pins apply)
+// chain length from which the lattice call uses the hash-map kernel: measured crossover with the O(N^2) scan kernel
+// (2^24 chains: N = 128 scan 26.8 ms / hash 42.8 ms; N = 256 scan 152 ms / hash 84 ms). ROSEN_LATTICE_HASH_MIN_N overrides
+// it in 2 .. 513 (tests run either kernel over the other's range; results do not depend on the choice).
 int32_t hash_min_n()
 {
     const char* e = std::getenv("ROSEN_LATTICE_HASH_MIN_N");
-    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_LATTICE_MAX_N) return (int32_t)v; }
-    return ROSEN_LATTICE_SCAN_MAX_N + 1;
+    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_LATTICE_SCAN_MAX_N + 1) return (int32_t)v; }
+    return ROSEN_LATTICE_HASH_MIN_N;
 }
 
 // same for the real-space call (cell-list kernel, realspace_long.cu); ROSEN_REALSPACE_CELL_MIN_N overrides it

@@ -53,8 +53,6 @@ __device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t entries)
     return __umulhi((uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> 32), entries);
 }
 
-__device__ __forceinline__ ulonglong2 load_entry(const ulonglong2* table, uint32_t slot) { return table[slot]; }
-
 // three-way select by axis
 template <typename T> __device__ __forceinline__ T pick(uint32_t a, T v0, T v1, T v2) { return a == 0u ? v0 : (a == 1u ? v1 : v2); }
 

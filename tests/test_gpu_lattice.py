@@ -89,13 +89,30 @@ def test_long_chains_hash_kernel(R, N, n_chains, seed, offset):
             assert s[k] == s2[k], k
 
 
+def test_scan_kernel_over_its_whole_range(R, monkeypatch):
+    """By default N >= ROSEN_LATTICE_HASH_MIN_N = 193 takes the hash-map kernel; ROSEN_LATTICE_HASH_MIN_N=513 keeps the
+    scan kernel up to its limit N = 512 so that its wide variant stays covered against the oracle."""
+    monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "513")
+    for N, n, seed in [(193, 800, 12), (256, 1200, 11), (300, 300, 13), (512, 200, 14)]:
+        s, t = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
+        assert "lattice_dp_kernel<wide" in R.rosen_last_kernel_name()
+        o = oracle.lattice_generate(N, n, seed)
+        compare_per_chain(t, o, N)
+        compare_summary(s, o.summary)
+    monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N")
+    R.rosen_lattice_generate(192, 100, 1)
+    assert "lattice_dp_kernel" in R.rosen_last_kernel_name()
+    R.rosen_lattice_generate(193, 100, 1)
+    assert "lattice_hash_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 3
+
+
 def test_hash_kernel_equals_scan_kernel_on_short_chains(R, monkeypatch):
     """ROSEN_LATTICE_HASH_MIN_N routes short chains through the hash kernel: it must reproduce the scan kernel
     (and with it the oracle and its enumeration pins) bit for bit, per chain and in the ensemble sums, with
     many chains per lane (table generations) and more chains than resident threads."""
     import torch
     for N, n, seed in [(16, 1 << 16, 1), (64, 400000, 7), (200, 30011, 3)]:
-        monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N", raising=False)
+        monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "513")
         s_scan, t_scan = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
         assert "lattice_dp_kernel" in R.rosen_last_kernel_name()
         monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "2")
@@ -241,7 +258,10 @@ def test_config4_sweep_reduced(R):
     for N in workloads.CONFIG_4_N:
         s, t = R.rosen_lattice_generate(N, n, 11, outputs=("digest", "lnW", "alive", "ree2"))
         name = R.rosen_last_kernel_name()
-        assert name.startswith("lattice_dp_kernel<wide") if N > 64 else name.startswith("lattice_dp_kernel") and "wide" not in name
+        if N >= 193:
+            assert name.startswith("lattice_hash_kernel")
+        else:
+            assert name.startswith("lattice_dp_kernel<wide") if N > 64 else name.startswith("lattice_dp_kernel") and "wide" not in name
         pre = 384
         o = oracle.lattice_generate(N, pre, 11, outputs=("digest", "lnW", "alive", "ree2"))
         assert np.array_equal(t["digest"][:pre].cpu().numpy().view(np.uint64), o.digest)
