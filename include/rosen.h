@@ -50,8 +50,9 @@ extern "C" {
 #define ROSEN_LATTICE_HASH_MIN_N 193  /* from here on the hash-map kernel is faster and is used (measured crossover)   */
 #define ROSEN_LATTICE_MAX_N  16383   /* beyond: per-chain hash set in HBM (lattice_hash.cu), the range of the paper's
                                         "global-memory version", Table 1 PAPER.md:282-288 (N = 100 ... 10000)        */
-#define ROSEN_REALSPACE_SCAN_MAX_N 2048  /* up to here: chain in shared memory (realspace.cu); the paper's longest
-                                           shared-memory chain, Table 2                                  */
+#define ROSEN_REALSPACE_SCAN_MAX_N 2048  /* longest chain of the shared-memory scan kernel (realspace.cu) = the paper's
+                                           longest shared-memory chain, Table 2                          */
+#define ROSEN_REALSPACE_CELL_MIN_N 400   /* from here on the cell-list kernel is faster and is used (measured crossover) */
 #define ROSEN_REALSPACE_MAX_N 16383     /* beyond: chain + cell list in HBM, one warp per chain (realspace_long.cu),
                                            the range of Table 2's "global-memory version" rows, PAPER.md:315-320      */
 
@@ -113,7 +114,7 @@ ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed
  * fma(bond_len, u_t, r_{s-1}); it overlaps if fma(dz,dz,fma(dy,dy,dx*dx)) < sigma*sigma (fp32)
  * for some j <= s-2; m_s = number of non-overlapping trials; the ((u_s*m_s)>>32)-th of them in
  * trial order is taken, u_s as in the lattice call. 2 <= N <= ROSEN_REALSPACE_MAX_N,
- * 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, both finite. N > ROSEN_REALSPACE_SCAN_MAX_N uses the library's
+ * 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, both finite. N >= ROSEN_REALSPACE_CELL_MIN_N uses the library's
  * long-chain workspace like the lattice call.
  */
 ROSEN_API int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,

@@ -82,12 +82,14 @@ int32_t hash_min_n()
     return ROSEN_LATTICE_HASH_MIN_N;
 }
 
-// same for the real-space call (cell-list kernel, realspace_long.cu); ROSEN_REALSPACE_CELL_MIN_N overrides it
+// same for the real-space call (cell-list kernel, realspace_long.cu): measured crossover with the shared-memory scan
+// kernel between N = 340 (k = 16) and N = 470 (k = 64); at N = 2048 the cell list is 10x faster. ROSEN_REALSPACE_CELL_MIN_N
+// overrides it in 2 .. 2049.
 int32_t cell_min_n()
 {
     const char* e = std::getenv("ROSEN_REALSPACE_CELL_MIN_N");
-    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_REALSPACE_MAX_N) return (int32_t)v; }
-    return ROSEN_REALSPACE_SCAN_MAX_N + 1;
+    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_REALSPACE_SCAN_MAX_N + 1) return (int32_t)v; }
+    return ROSEN_REALSPACE_CELL_MIN_N;
 }
 
 struct Sizes { size_t lnW, alive, m_seq, digest, conf, ree2, rg2; };

@@ -78,6 +78,20 @@ def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
     check(R, N, n, k, b, sigma, seed, offset)
 
 
+def test_scan_kernel_over_its_whole_range(R, monkeypatch):
+    """By default N >= ROSEN_REALSPACE_CELL_MIN_N = 400 takes the cell-list kernel; ROSEN_REALSPACE_CELL_MIN_N=2049 keeps
+    the shared-memory scan kernel up to its limit so that its long-chain variants stay covered against the oracle."""
+    monkeypatch.setenv("ROSEN_REALSPACE_CELL_MIN_N", "2049")
+    for args in [(400, 20, 16, 1.0, 1.0, 13, 0), (1024, 6, 4, 1.0, 0.6, 15, 0), (1024, 3, 2, 0.5, 0.0, 15, 2), (2048, 3, 3, 1.0, 0.5, 16, 1)]:
+        check(R, *args)
+        assert R.rosen_last_kernel_name().startswith("realspace_kernel")
+    monkeypatch.delenv("ROSEN_REALSPACE_CELL_MIN_N")
+    R.rosen_realspace_generate(399, 10, 4, 1.0, 0.5, 1)
+    assert R.rosen_last_kernel_name().startswith("realspace_kernel")
+    R.rosen_realspace_generate(400, 10, 4, 1.0, 0.5, 1)
+    assert R.rosen_last_kernel_name().startswith("realspace_long_kernel") and R.rosen_last_launch_count() == 3
+
+
 # Long chains (N > ROSEN_REALSPACE_SCAN_MAX_N = 2048): the cell-list kernel of realspace_long.cu, the range of the
 # paper's real-space "global-memory version" (Table 2, PAPER.md:315-320). Same bars as the shared-memory kernel.
 @pytest.mark.parametrize("N,n,k,b,sigma,seed,offset", [
