@@ -48,16 +48,16 @@ __device__ __forceinline__ uint64_t cell_key(int cx, int cy, int cz)
 }
 
 // R2 for one batch of candidates: every trial of this lane against cand[0..n)
-template <int P>
-__device__ __forceinline__ void test_batch(const float4* cand, int n, const float (&tx)[P][2], const float (&ty)[P][2],
-                                           const float (&tz)[P][2], bool (&fr)[P][2], float sigma2)
+template <int PP, int E>
+__device__ __forceinline__ void test_batch(const float4* cand, int n, const float (&tx)[PP][E], const float (&ty)[PP][E],
+                                           const float (&tz)[PP][E], bool (&fr)[PP][E], float sigma2)
 {
     for (int c = 0; c < n; ++c) {
         const float4 rj = cand[c];
 #pragma unroll
-        for (int pp = 0; pp < P; ++pp)
+        for (int pp = 0; pp < PP; ++pp)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
+            for (int e = 0; e < E; ++e) {
                 const float dx = __fsub_rn(rj.x, tx[pp][e]), dy = __fsub_rn(rj.y, ty[pp][e]), dz = __fsub_rn(rj.z, tz[pp][e]);
                 const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                 if (d2 < sigma2) fr[pp][e] = false;
@@ -65,9 +65,12 @@ __device__ __forceinline__ void test_batch(const float4* cand, int n, const floa
     }
 }
 
+// P = Philox blocks (trial pairs) per lane: lane owns trials 2 (lane + 32 pp) + {0, 1}. P = 0 (k <= 32): ONE trial per lane,
+// trial t = lane from block lane >> 1 (the pair's two lanes draw the same block), so that 16 trials keep 16 lanes busy.
 template <int P, bool DIGEST, bool TRAJ>
 __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(const RealLongParams p)
 {
+    constexpr int PP = P == 0 ? 1 : P, E = P == 0 ? 1 : 2;
     __shared__ double ln_tab[256];
     __shared__ float4 cand_all[kWarpsPerBlock][kCandCap];
     for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
@@ -119,21 +122,22 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
             const uint32_t usel = (s & 2) ? ((s & 1) ? selw[3] : selw[2]) : ((s & 1) ? selw[1] : selw[0]);
 
             // ---- R1: this lane's trials (P Philox blocks = 2P trials), trial index t = 2 (lane + 32 pp) + e
-            float tx[P][2], ty[P][2], tz[P][2];
-            bool fr[P][2];
+            float tx[PP][E], ty[PP][E], tz[PP][E];
+            bool fr[PP][E];
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp) {
-                const uint32_t bi = (uint32_t)(lane + 32 * pp);
+            for (int pp = 0; pp < PP; ++pp) {
+                const uint32_t bi = P == 0 ? (uint32_t)lane >> 1 : (uint32_t)(lane + 32 * pp);
                 uint32_t w[4];
                 philox4x32_10(c_lo, c_hi, (uint32_t)s, 1u + bi, p.key0, p.key1, w);
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
+                for (int e = 0; e < E; ++e) {
+                    const bool second = P == 0 ? (lane & 1) != 0 : e != 0;       // which trial of the pair
                     float ux, uy, uz;
-                    direction(w[2 * e], w[2 * e + 1], ux, uy, uz);
+                    direction(second ? w[2] : w[0], second ? w[3] : w[1], ux, uy, uz);
                     tx[pp][e] = __fmaf_rn(p.b, ux, hx);
                     ty[pp][e] = __fmaf_rn(p.b, uy, hy);
                     tz[pp][e] = __fmaf_rn(p.b, uz, hz);
-                    fr[pp][e] = (int)(2u * bi + e) < k;
+                    fr[pp][e] = (int)(2u * bi + (second ? 1u : 0u)) < k;
                 }
             }
 
@@ -167,21 +171,21 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
                 ncand += __popc(bal);
                 if (ncand > (int)p.cand_cap - 32) {    // buffer may not hold another round: test what is there
                     __syncwarp();
-                    test_batch<P>(cand, ncand, tx, ty, tz, fr, p.sigma2);
+                    test_batch<PP, E>(cand, ncand, tx, ty, tz, fr, p.sigma2);
                     ncand = 0;
                     __syncwarp();
                 }
             }
             __syncwarp();
-            test_batch<P>(cand, ncand, tx, ty, tz, fr, p.sigma2);
+            test_batch<PP, E>(cand, ncand, tx, ty, tz, fr, p.sigma2);
 
             // ---- m_s and the rank of each free trial in trial order
-            uint32_t B[P][2];
+            uint32_t B[PP][E];
             uint32_t m = 0;
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp)
+            for (int pp = 0; pp < PP; ++pp)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
+                for (int e = 0; e < E; ++e) {
                     B[pp][e] = __ballot_sync(0xffffffffu, fr[pp][e]);
                     m += __popc(B[pp][e]);
                 }
@@ -191,19 +195,23 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
             if (m == 0u) { dead = (uint32_t)s; if (DIGEST) dg = digest_fold(dg, 0u, 0xFFu); break; }
             lnW += ln_tab[m];
 
-            // ---- R4: the sel-th free trial becomes r_s
+            // ---- R4: the sel-th free trial (in trial order) becomes r_s
             const uint32_t sel = __umulhi(usel, m);
             uint32_t rank0 = 0;
             bool hit = false;
             float px = hx, py = hy, pz = hz;
             uint32_t tsel = 0;
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp) {
-                const uint32_t r0 = rank0 + __popc(B[pp][0] & below) + __popc(B[pp][1] & below);
-                const uint32_t r1 = r0 + (fr[pp][0] ? 1u : 0u);
-                if (fr[pp][0] && r0 == sel) { hit = true; px = tx[pp][0]; py = ty[pp][0]; pz = tz[pp][0]; tsel = 2u * (lane + 32 * pp); }
-                if (fr[pp][1] && r1 == sel) { hit = true; px = tx[pp][1]; py = ty[pp][1]; pz = tz[pp][1]; tsel = 2u * (lane + 32 * pp) + 1u; }
-                rank0 += __popc(B[pp][0]) + __popc(B[pp][1]);
+            for (int pp = 0; pp < PP; ++pp) {
+                if (P == 0) {
+                    if (fr[0][0] && (uint32_t)__popc(B[0][0] & below) == sel) { hit = true; px = tx[0][0]; py = ty[0][0]; pz = tz[0][0]; tsel = (uint32_t)lane; }
+                } else {
+                    const uint32_t r0 = rank0 + __popc(B[pp][0] & below) + __popc(B[pp][E - 1] & below);
+                    const uint32_t r1 = r0 + (fr[pp][0] ? 1u : 0u);
+                    if (fr[pp][0] && r0 == sel) { hit = true; px = tx[pp][0]; py = ty[pp][0]; pz = tz[pp][0]; tsel = 2u * (lane + 32 * pp); }
+                    if (fr[pp][E - 1] && r1 == sel) { hit = true; px = tx[pp][E - 1]; py = ty[pp][E - 1]; pz = tz[pp][E - 1]; tsel = 2u * (lane + 32 * pp) + 1u; }
+                    rank0 += __popc(B[pp][0]) + __popc(B[pp][E - 1]);
+                }
             }
             const uint32_t hb = __ballot_sync(0xffffffffu, hit);
             const int src = __ffs(hb) - 1;
@@ -289,7 +297,8 @@ int real_long_max_warps(int k, int* warps_out)
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
     cudaError_t e;
-    if (k <= 64)       e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, realspace_long_kernel<1, true, true>, 32 * kWarpsPerBlock, 0);
+    if (k <= 32)       e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, realspace_long_kernel<0, true, true>, 32 * kWarpsPerBlock, 0);
+    else if (k <= 64)  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, realspace_long_kernel<1, true, true>, 32 * kWarpsPerBlock, 0);
     else if (k <= 128) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, realspace_long_kernel<2, true, true>, 32 * kWarpsPerBlock, 0);
     else               e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, realspace_long_kernel<4, true, true>, 32 * kWarpsPerBlock, 0);
     if (e != cudaSuccess || per_sm < 1) return -3;
@@ -300,7 +309,8 @@ int real_long_max_warps(int k, int* warps_out)
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name)
 {
     int rc;
-    if (p.k <= 64)       { *kernel_name = "realspace_long_kernel<P=1>"; rc = launch_p<1>(p, n_warps, stream); }
+    if (p.k <= 32)       { *kernel_name = "realspace_long_kernel<P=1/2>"; rc = launch_p<0>(p, n_warps, stream); }
+    else if (p.k <= 64)  { *kernel_name = "realspace_long_kernel<P=1>"; rc = launch_p<1>(p, n_warps, stream); }
     else if (p.k <= 128) { *kernel_name = "realspace_long_kernel<P=2>"; rc = launch_p<2>(p, n_warps, stream); }
     else                 { *kernel_name = "realspace_long_kernel<P=4>"; rc = launch_p<4>(p, n_warps, stream); }
     if (rc < 0) return rc;
