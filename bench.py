@@ -47,7 +47,7 @@ def lattice_site_tests(N: int) -> int:
     return sum(max(0, s // 2 - 1) for s in range(1, N))
 
 
-HASH_INSTR_PER_STEP = 123.5     # long lattice chains (N > 512), per attempted step; see run_product
+HASH_INSTR_PER_STEP = 123.5     # hash-map lattice kernel (N >= 193), per attempted step; see run_product
 
 
 def algorithmic_thread_instr(w: workloads.Workload) -> float:
@@ -343,14 +343,14 @@ def run_product(args, w, rank, world, local_rank):
     peak_winst = n_sm * 4 * sm_hz                           # 4 schedulers/SM, 1 warp-instruction/clk each
     alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
     achieved = alg_winst / (kernel_ms * 1e-3)
-    if w.kind == "lattice" and w.N > 512:
+    if w.kind == "lattice" and w.N >= 193:
         # hash-map kernel (DESIGN.md 5.5 / 6): ncu shows it issue-bound (59.6 % issue-active, 26 % of DRAM peak), so the
         # roofline is the issue peak; algorithmic work per ATTEMPTED step (not per nominal step: most long chains die
         # early): 3 cube look-ups (hash 8 + compare 6 each), 6 occupancy bits (4 each), count/choose 15, insert 10,
         # observables 12, weight 3, a quarter Philox block 17.5 = 123.5 thread-instructions
         alg_winst = HASH_INSTR_PER_STEP * (steps_attempted / world) / 32.0
         achieved = alg_winst / (kernel_ms * 1e-3)
-    long_real = w.kind == "realspace" and w.N > 2048
+    long_real = w.kind == "realspace" and w.N >= 400
     if long_real:
         # cell-list kernel (DESIGN.md 5.6 / 6), per ATTEMPTED step: k trials x (35 Philox + 45 direction + 7 x 3.2 candidate
         # pair tests) + 27 cell look-ups x 14 + ~40 listed monomers x 10 (candidate test) + 50 for count/choose/place/sums
@@ -361,7 +361,7 @@ def run_product(args, w, rank, world, local_rank):
                 "frac": achieved / peak_winst, "traffic": profile_traffic(w), "kernel": kernel_name, "kernel_ms": kernel_ms,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
                 "algorithmic_thread_instr_per_chain": algorithmic_thread_instr(w)}
-    if w.kind == "lattice" and w.N > 512:
+    if w.kind == "lattice" and w.N >= 193:
         del roofline["algorithmic_thread_instr_per_chain"]
         roofline["algorithmic_thread_instr_per_attempted_step"] = HASH_INSTR_PER_STEP
         roofline["note"] = "kernel_ms covers table memset + generation kernel + record reduction"

@@ -102,7 +102,9 @@ typedef struct rosen_outputs {
  * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
  * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N >= ROSEN_LATTICE_HASH_MIN_N the library keeps device
  * workspace (at most 12 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
- * rosen_workspace_release(); the results do not depend on which kernel ran.
+ * rosen_workspace_release(); the results do not depend on which kernel ran. That workspace is one per device:
+ * long-chain calls (lattice or real space) on the same device must not overlap in time, i.e. enqueue them on one stream
+ * or synchronise between streams / host threads.
  */
 ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
                            const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
