@@ -46,10 +46,12 @@ def test_shard_ranges_cover_population():
             assert o1 + c1 == o2
 
 
-def test_two_rank_gloo_merge_equals_single_range():
+@pytest.mark.parametrize("N,n_total,seed", [(16, 4001, 5), (700, 301, 9)])
+def test_two_rank_gloo_merge_equals_single_range(N, n_total, seed):
+    """(16, ...): equal fixed shifts. (700, ...): a long chain length, where every rank's shift is the largest lnW of its
+    own range (reading A18) and rosen_summary_merge rescales the parts to the larger one."""
     import torch.multiprocessing as mp
     import oracle
-    N, n_total, seed = 16, 4001, 5        # odd population: ragged shards
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = _free_port()
