@@ -66,7 +66,8 @@ def profile_traffic(w: workloads.Workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu summary of
     this workload (profiles/), per launch; None if no capture is committed."""
     name = {"lattice_N64_2p24": "r01d_lattice_cfg2.md", "realspace_N64_k16_2p22": "r01d_realspace_cfg3.md",
-            "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md"}.get(w.name)
+            "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md",
+            "realspace_long_N4096_k16_2p16": "r01e_realspace_long_N4096.md"}.get(w.name)
     path = os.path.join(ROOT, "profiles", name) if name else None
     if not path or not os.path.exists(path):
         return None
