@@ -56,11 +56,17 @@ __device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t entries)
 // three-way select by axis
 template <typename T> __device__ __forceinline__ T pick(uint32_t a, T v0, T v1, T v2) { return a == 0u ? v0 : (a == 1u ? v1 : v2); }
 
-template <bool TRAJ>
+template <bool TRAJ, bool DIGEST>
 __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p)
 {
     __shared__ double ln_m[8];
+    __shared__ uint8_t nth_free[64 * 8];    // [free-direction mask][sel] -> the sel-th free direction, order +x,-x,+y,-y,+z,-z
     if (threadIdx.x < 8) ln_m[threadIdx.x] = threadIdx.x == 0 ? -CUDART_INF : log((double)threadIdx.x);
+    for (uint32_t i = threadIdx.x; i < 64u * 8u; i += blockDim.x) {
+        uint32_t fr = i >> 3;
+        for (uint32_t k = 0; k < (i & 7u); ++k) fr &= fr - 1u;
+        nth_free[i] = (uint8_t)(fr ? __ffs((int)fr) - 1 : 0);
+    }
     __syncthreads();
 
     const int N = p.N;
@@ -165,15 +171,15 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
         bool done;
         if (m == 0u) {
             // ---- L3: dead end (W = 0, chain kept; reading A6)
-            dg = digest_fold(dg, 0u, 0xFFu);
+            if (DIGEST) dg = digest_fold(dg, 0u, 0xFFu);
             done = true;
         } else {
             lnW += ln_m[m];
             // ---- L4
             const uint32_t u = (s & 2) ? ((s & 1) ? w[3] : w[2]) : ((s & 1) ? w[1] : w[0]);
             const uint32_t sel = __umulhi(u, m);
-            const uint32_t d = __fns(~occ & 63u, 0u, (int)sel + 1);       // sel-th free direction in the order +x,-x,+y,-y,+z,-z
-            dg = digest_fold(dg, m, d);
+            const uint32_t d = nth_free[((~occ & 63u) << 3) + sel];
+            if (DIGEST) dg = digest_fold(dg, m, d);
             const uint32_t a = d >> 1;
             const bool up = (d & 1u) == 0u;
             const uint32_t la = (l >> (2u * a)) & 3u;
@@ -210,7 +216,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             }
             r.steps = alive ? (uint32_t)(N - 1) : (uint32_t)s;     // attempted steps
             r.alive = alive ? 1u : 0u;
-            r.digest = dg;
+            r.digest = DIGEST ? dg : 0ull;
             p.rec[idx] = r;
             s = 0;
         }
@@ -293,7 +299,7 @@ int hash_max_threads(int* threads_out)
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
     // the traj variant has the larger register footprint: size the tables for the plain one, which every launch may use
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lattice_hash_kernel<false>, 256, 0) != cudaSuccess || per_sm < 1) return -3;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lattice_hash_kernel<false, false>, 256, 0) != cudaSuccess || per_sm < 1) return -3;
     if (const char* e = std::getenv("ROSEN_HASH_BLOCKS_PER_SM")) {     // tuning knob (results do not depend on it)
         const int v = std::atoi(e);
         if (v >= 1 && v < per_sm) per_sm = v;
@@ -306,8 +312,14 @@ int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream,
 {
     const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
     const int grid = n_threads / 256;
-    if (traj) { *kernel_name = "lattice_hash_kernel<traj>"; lattice_hash_kernel<true><<<grid, 256, 0, stream>>>(p); }
-    else      { *kernel_name = "lattice_hash_kernel";       lattice_hash_kernel<false><<<grid, 256, 0, stream>>>(p); }
+    const bool digest = p.out.digest != nullptr;
+    if (traj) {
+        if (digest) { *kernel_name = "lattice_hash_kernel<digest,traj>"; lattice_hash_kernel<true, true><<<grid, 256, 0, stream>>>(p); }
+        else        { *kernel_name = "lattice_hash_kernel<traj>";        lattice_hash_kernel<true, false><<<grid, 256, 0, stream>>>(p); }
+    } else {
+        if (digest) { *kernel_name = "lattice_hash_kernel<digest>";      lattice_hash_kernel<false, true><<<grid, 256, 0, stream>>>(p); }
+        else        { *kernel_name = "lattice_hash_kernel";              lattice_hash_kernel<false, false><<<grid, 256, 0, stream>>>(p); }
+    }
     if (cudaGetLastError() != cudaSuccess) return -3;
     const int rc = launch_reduce_records(p.rec, p.n_chains, p.chunk, p.n_vblocks, p.ln_shift, p.lmax, p.out, p.partials, stream);
     return rc < 0 ? rc : 1 + rc;
