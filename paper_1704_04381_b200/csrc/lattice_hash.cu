@@ -140,20 +140,30 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             nslot[a] = need[a] ? slot_of(nkey[a], entries) : slot;
             first[a] = table[nslot[a]];
         }
+        uint32_t pend = 0;
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            const uint64_t want = nkey[a] | tag;
-            const bool hit = first[a].x == want;
+            const bool hit = first[a].x == (nkey[a] | tag);
             nbits[a] = hit ? first[a].y : 0ull;
-            if (need[a] && (uint32_t)(first[a].x >> kGenShift) == gen && !hit) {
-                // home entry taken by another cube of this chain (rare: tables are at most ~1/6 full on average)
-                for (;;) {
-                    nslot[a] = nslot[a] + 1u == entries ? 0u : nslot[a] + 1u;
-                    const ulonglong2 e = table[nslot[a]];
-                    if ((uint32_t)(e.x >> kGenShift) != gen) break;                    // empty: cube not visited yet; nslot = where it would go
-                    if (e.x == want) { nbits[a] = e.y; break; }
-                }
+            pend |= (need[a] && (uint32_t)(first[a].x >> kGenShift) == gen && !hit) ? 1u << a : 0u;
+        }
+        while (pend) {
+            // home entry taken by another cube of this chain (tables are ~1/6 full at most on average): one shared
+            // probe loop for whichever axes need it
+            const uint32_t a = (uint32_t)__ffs((int)pend) - 1u;
+            pend &= pend - 1u;
+            const uint64_t want = pick(a, nkey[0], nkey[1], nkey[2]) | tag;
+            uint32_t sl = pick(a, nslot[0], nslot[1], nslot[2]);
+            uint64_t nb = 0ull;
+            for (;;) {
+                sl = sl + 1u == entries ? 0u : sl + 1u;
+                const ulonglong2 e = table[sl];
+                if ((uint32_t)(e.x >> kGenShift) != gen) break;                    // empty: cube not visited yet; sl = where it would go
+                if (e.x == want) { nb = e.y; break; }
             }
+            if (a == 0u) { nslot[0] = sl; nbits[0] = nb; }
+            if (a == 1u) { nslot[1] = sl; nbits[1] = nb; }
+            if (a == 2u) { nslot[2] = sl; nbits[2] = nb; }
         }
         uint32_t occ = 0;
 #pragma unroll
