@@ -447,6 +447,63 @@ def run_sweep(args):
                       "sweep": rows, "data": "synthetic"}))
 
 
+# The paper's own benchmark (Tables 1-2): wall time to generate 10^6 chains of N monomers, for the lengths its
+# tables list. Its chains are restarted on dead ends, so its times are per 10^6 FULL-LENGTH chains; here dead chains are kept
+# (reading A6), so both the time per 10^6 attempts and that time divided by the surviving fraction are reported.
+PAPER_TABLE_N = (4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 100, 500, 1000, 2500, 5000, 10000)
+PAPER_TABLE1_GTX1080_S = {4: 0.00324, 8: 0.00901, 16: 0.02664, 32: 0.09192, 64: 0.38830, 128: 1.73263, 256: 7.50125, 512: 49.8232,
+                          1024: 373.824, 2048: 3981.55, 100: 8.1, 500: 14.5, 1000: 559.9, 2500: 3574.0, 5000: 14088.0, 10000: 55883.1}
+PAPER_TABLE2_GTX1080_S = {4: 0.16288, 8: 0.44877, 16: 2.31603, 32: 11.4375, 64: 58.3319, 128: 226.441, 256: 986.501, 512: 5905.82,
+                          1024: 45513.8, 2048: 378758.0}
+
+
+def run_paper_tables(args):
+    """`--paper-tables`: 10^6 chains per length of Tables 1-2 (lattice; real space with k = 16, b = sigma = 1 -- the paper
+    does not state its trial set -- and with k = 64, sigma = 0.8 for the long lengths where the former lets no chain
+    survive). One JSON line; times are device-timed, best of 3, summary-only calls."""
+    import torch
+    import paper_1704_04381_b200 as R
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    R.load_library()
+    stream = torch.cuda.Stream()
+    summary_dev = torch.zeros(R.SUMMARY_BYTES, dtype=torch.uint8, device="cuda")
+    n = 1000000
+
+    def timed(call):
+        ev = []
+        with torch.cuda.stream(stream):
+            for _ in range(4):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); call(); b.record(stream)
+                ev.append((a, b))
+        stream.synchronize()
+        return min(a.elapsed_time(b) for a, b in ev[1:]) * 1e-3
+
+    def row(N, sec, paper):
+        sm = R.summary_from_device(summary_dev)
+        alive = 1.0 - sm["attrition"]
+        return {"N": N, "s_per_1e6_attempts": sec, "alive_fraction": alive,
+                "s_per_1e6_full_length": sec / alive if alive > 0 else None, "paper_gtx1080_s": paper,
+                "monomer_steps_per_s": sm["n_steps_attempted"] / sec, "kernel": R.rosen_last_kernel_name()}
+
+    lattice, real16, real64 = [], [], []
+    for N in PAPER_TABLE_N:
+        sec = timed(lambda: R.rosen_lattice_generate_async(N, n, 1, 0, outputs=None, summary_device=summary_dev, stream=stream))
+        lattice.append(row(N, sec, PAPER_TABLE1_GTX1080_S.get(N)))
+    for N in PAPER_TABLE_N:
+        sec = timed(lambda: R.rosen_realspace_generate_async(N, n, 16, 1.0, 1.0, 1, 0, outputs=None, summary_device=summary_dev, stream=stream))
+        real16.append(row(N, sec, PAPER_TABLE2_GTX1080_S.get(N)))
+    for N in (512, 1024, 2048, 2500, 5000, 10000):
+        m = n // 10                                                    # 10^5 chains, scaled to 10^6
+        sec = timed(lambda: R.rosen_realspace_generate_async(N, m, 64, 1.0, 0.8, 1, 0, outputs=None, summary_device=summary_dev, stream=stream))
+        r = row(N, sec * 10.0, PAPER_TABLE2_GTX1080_S.get(N))
+        r["note"] = "10^5 chains timed, x10"
+        real64.append(r)
+    print(json.dumps({"metric": "seconds per 10^6 chains at the lengths of the paper's Tables 1-2 (PAPER.md:266-320)", "n_chains": n,
+                      "lattice": lattice, "realspace_k16_sigma1": real16, "realspace_k64_sigma0.8": real64, "data": "synthetic"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -457,6 +514,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE config 4 (length sweep) instead")
+    ap.add_argument("--paper-tables", action="store_true", help="10^6 chains at every length of the paper's Tables 1-2 instead")
     args = ap.parse_args()
     w = workloads.CONFIGS[args.workload]
     rank = int(os.environ.get("RANK", "0"))
@@ -465,6 +523,10 @@ def main():
     if args.sweep:
         if rank == 0:
             run_sweep(args)
+        return
+    if args.paper_tables:
+        if rank == 0:
+            run_paper_tables(args)
         return
     if args.impl == "reference":
         run_reference(args, w, rank)
