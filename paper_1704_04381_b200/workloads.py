@@ -39,7 +39,8 @@ CONFIG_5 = Workload("realspace_N256_k64_2p20_dump", "realspace", 256, 1 << 20, 1
 # N = 1024 / 2048 of the shared-memory rows and N = 10000, the longest "global-memory version" row.
 LONG_LATTICE = (Workload("lattice_long_N1024_2p20", "lattice", 1024, 1 << 20, 17),
                 Workload("lattice_long_N2048_2p19", "lattice", 2048, 1 << 19, 17),
-                Workload("lattice_long_N10000_2p17", "lattice", 10000, 1 << 17, 17))
+                Workload("lattice_long_N10000_2p17", "lattice", 10000, 1 << 17, 17),      # 1.7 chains per resident thread: tail-dominated
+                Workload("lattice_long_N10000_2p20", "lattice", 10000, 1 << 20, 17))
 
 # ... and of Table 2; the paper does not state its trial set: config 3's (k = 16, b = sigma = 1,
 # where 96 % of the chains die before N = 4096) and config 5's (k = 64, sigma = 0.8, where nearly all reach N = 10000).
