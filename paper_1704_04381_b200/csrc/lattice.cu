@@ -8,7 +8,7 @@
 // neighbour keys: it classifies w = key_j - h (an integer, because the fields cannot borrow into each other for
 // chains this short) with a byte dot product on the tensor-free IDP.4A path and XOR-accumulates the neighbours'
 // w (half of the keys select by a clamped shift, half by a predicate: that balances the alu and fma-heavy pipes)
-// -- about 5.25 issue slots per key (N <= 64) or 7.25 (N <= 512) instead of 6 half-rate ISETP.
+// -- about 5.25 issue slots per key (N <= 128) or 7.25 (N <= 512) instead of 6 half-rate ISETP.
 #include <algorithm>
 #include <math_constants.h>
 #include "common.cuh"
@@ -31,8 +31,9 @@ __host__ __device__ inline int half4_of(int N) { return (((N + 1) / 2) + 3) & ~3
 __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 
 // =====================================================================================================
-// N <= 64: the byte-dot-product scan. Keys are plain integers with three 8-bit fields
-// biased by 128, so w = key_j - h is the integer dx + 256 dy + 65536 dz with |d| <= 126 < 2^7, a unique
+// N <= 128: the byte-dot-product scan. Keys are plain integers with three 8-bit fields
+// biased by 128 (|coordinate| <= 127), and the scan at step s only meets monomers j <= s-2 <= 125 bonds away from
+// the growth point, so w = key_j - h is the integer dx + 256 dy + 65536 dz with |d| <= 126 < 2^7, a unique
 // balanced representation: monomer j sits on a neighbour site of h iff |w| is 1, 2^8 or 2^16, i.e. iff
 // exactly one byte of |w| is 1 and the rest are 0 (|w| < 2^24), i.e. iff dp4a.u8(|w|, |w|) == 1. The
 // scan XOR-accumulates w over those keys without a predicate: d = dp4a(|w|,|w|,-1) is 0 for a
@@ -113,7 +114,7 @@ __device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t 
     return A;
 }
 
-// 64 < N <= 512: 10-bit fields. |w| is 1, 2^10 or 2^20 iff z = |w| & ((|w| - 1) | ~M) is 0 (power of two inside
+// 128 < N <= 512: 10-bit fields. |w| is 1, 2^10 or 2^20 iff z = |w| & ((|w| - 1) | ~M) is 0 (power of two inside
 // M = 2^0 | 2^10 | 2^20; |w| = 0 cannot occur: sites are distinct and an empty slot gives |w| = h). d = byte sum of z
 // (IDP.4A against 0x01010101) is 0 for a neighbour and >= 1 otherwise; the rest is as in scan_dp.
 #define ROSEN_DPW_CHUNK(W)                                                                           \
@@ -166,9 +167,14 @@ __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts128(uint32_t a, uint32_t v) { asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" :: "r"(a), "r"(v), "r"(0u) : "memory"); }
 
-template <bool WIDE, bool DIGEST, bool TRAJ>
+// MODE 0: N <= 64, 8-bit fields, lnW from an m histogram. MODE 1: 64 < N <= 128, 8-bit fields, lnW as a running fp64 sum in
+// step order (lnW crosses 128 there, where the oracle's step-by-step sum rounds every ln 5 it adds the same way -- a systematic
+// 6e-13 relative to the histogram's more accurate value; following the oracle's order keeps the ensemble sums within 1e-13).
+// MODE 2 ("wide"): 128 < N <= 512, 10-bit fields, running sum.
+template <int MODE, bool DIGEST, bool TRAJ>
 __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
 {
+    constexpr bool WIDE = MODE == 2, RUNSUM = MODE >= 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     DpTables* tab = reinterpret_cast<DpTables*>(smem_raw);
     Partial* scratch = reinterpret_cast<Partial*>(smem_raw + sizeof(DpTables));
@@ -206,12 +212,13 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
             const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
 
             // L0. No clearing pass: the first key of every 4-key chunk is stored as {key, 0, 0, 0}, so a scan
-            // never sees a key of the previous chain (0 is not a neighbour of any head: |0 - h| >= 0x414141).
+            // never sees a key of the previous chain (0 is not a neighbour of any head: every byte of h is >= 1, so
+            // |0 - h| >= 0x010101 has at least two nonzero bytes).
             uint32_t h = kOrigin;
             sts128(ev_addr, h);
             int sx = 0, sy = 0, sz = 0, s2 = 0;
             uint32_t hist = 0, dead = 0;     // dead = step of the first m = 0 (0: alive)
-            double lnW_w = 0.0;             // WIDE: running sum (counts can exceed the 8-bit histogram)
+            double lnW_w = 0.0;             // RUNSUM: running sum in step order
             uint64_t dg = 0xCBF29CE484222325ull;
             uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
 
@@ -235,7 +242,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                     const uint32_t m = le.x & 7u;
 
                     // L3
-                    if (WIDE) lnW_w += tab->ln_m[m]; else hist += le.y;
+                    if (RUNSUM) lnW_w += tab->ln_m[m]; else hist += le.y;
                     if (TRAJ && mrow) mrow[s - 1] = dead == 0u ? (uint8_t)m : (uint8_t)0;
 
                     // L4
@@ -267,7 +274,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
             lnW += (double)((hist >> 8) & 255u) * tab->ln_m[3];
             lnW += (double)((hist >> 16) & 255u) * tab->ln_m[4];
             lnW += (double)(hist >> 24) * tab->ln_m[5];
-            if (WIDE) lnW = lnW_w;
+            if (RUNSUM) lnW = lnW_w;
             if (!alive) lnW = -CUDART_INF;
             double ree2 = 0.0, rg2 = 0.0;
             if (alive) {
@@ -330,16 +337,16 @@ int launch_kernel(Kern kern, size_t table_bytes, const LatticeParams& p, cudaStr
     return 1;
 }
 
-template <bool WIDE>
+template <int MODE>
 int launch_dp(const LatticeParams& p, cudaStream_t stream, int* grid_out)
 {
     const bool digest = p.out.digest != nullptr;
     const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
     const size_t tb = sizeof(DpTables);
-    if (traj) return digest ? launch_kernel(lattice_dp_kernel<WIDE, true, true>, tb, p, stream, grid_out)
-                            : launch_kernel(lattice_dp_kernel<WIDE, false, true>, tb, p, stream, grid_out);
-    return digest ? launch_kernel(lattice_dp_kernel<WIDE, true, false>, tb, p, stream, grid_out)
-                  : launch_kernel(lattice_dp_kernel<WIDE, false, false>, tb, p, stream, grid_out);
+    if (traj) return digest ? launch_kernel(lattice_dp_kernel<MODE, true, true>, tb, p, stream, grid_out)
+                            : launch_kernel(lattice_dp_kernel<MODE, false, true>, tb, p, stream, grid_out);
+    return digest ? launch_kernel(lattice_dp_kernel<MODE, true, false>, tb, p, stream, grid_out)
+                  : launch_kernel(lattice_dp_kernel<MODE, false, false>, tb, p, stream, grid_out);
 }
 
 }  // namespace
@@ -348,15 +355,15 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
 {
     const bool digest = p.out.digest != nullptr;
     const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
-    if (p.N <= 64) {    // |dx|,|dy|,|dz| <= 126 fit signed bytes: byte-dot-product scan
+    if (p.N <= 128) {   // every scanned difference |dx|,|dy|,|dz| <= s-1-j <= 126 fits a signed byte: byte-dot-product scan
         *kernel_name = traj ? (digest ? "lattice_dp_kernel<digest,traj>" : "lattice_dp_kernel<traj>")
                             : (digest ? "lattice_dp_kernel<digest>" : "lattice_dp_kernel");
-        return launch_dp<false>(p, stream, grid_out);
+        return p.N <= 64 ? launch_dp<0>(p, stream, grid_out) : launch_dp<1>(p, stream, grid_out);
     }
-    // 10-bit fields (|d| <= 510 < 2^9, N <= 512): power-of-two test + byte-sum scan
+    // 10-bit fields (|d| <= 510 < 2^9, 128 < N <= 512): power-of-two test + byte-sum scan
     *kernel_name = traj ? (digest ? "lattice_dp_kernel<wide,digest,traj>" : "lattice_dp_kernel<wide,traj>")
                         : (digest ? "lattice_dp_kernel<wide,digest>" : "lattice_dp_kernel<wide>");
-    return launch_dp<true>(p, stream, grid_out);
+    return launch_dp<2>(p, stream, grid_out);
 }
 
 }  // namespace rosen

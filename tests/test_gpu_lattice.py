@@ -261,7 +261,7 @@ def test_config4_sweep_reduced(R):
         if N >= 193:
             assert name.startswith("lattice_hash_kernel")
         else:
-            assert name.startswith("lattice_dp_kernel<wide") if N > 64 else name.startswith("lattice_dp_kernel") and "wide" not in name
+            assert name.startswith("lattice_dp_kernel<wide") if N > 128 else name.startswith("lattice_dp_kernel") and "wide" not in name
         pre = 384
         o = oracle.lattice_generate(N, pre, 11, outputs=("digest", "lnW", "alive", "ree2"))
         assert np.array_equal(t["digest"][:pre].cpu().numpy().view(np.uint64), o.digest)
