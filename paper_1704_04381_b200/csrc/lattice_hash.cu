@@ -1,4 +1,4 @@
-// lattice_hash.cu -- cubic-lattice Rosenbluth generation for LONG chains (512 < N <= 16383), the range of the
+// lattice_hash.cu -- cubic-lattice Rosenbluth generation for LONG chains (193 <= N <= 16383), the range of the
 // paper's "global-memory version" (Table 1; Fig. 2b, :296) and of its longest shared-memory
 // rows (N = 1024, 2048, :280-281). Same steps L0-L5 and the same decisions as lattice.cu, but
 // the occupancy scan of Alg. 1 lines 13-17, which costs O(s) per step, is replaced by an
@@ -25,7 +25,7 @@
 // by reduce_records_kernel over virtual blocks in a fixed order (deterministic, grid independent, no float
 // atomics), which also writes the optional per-chain outputs, coalesced.
 //
-// Roofline: random sector traffic to HBM/L2, not issue slots (DESIGN.md 5.5 / 6).
+// Roofline: issue slots (ncu: 60 % issue-active, 28 % of DRAM peak; the first per-site version was DRAM bound), DESIGN.md 5.5 / 6.
 #include <cstdlib>
 #include <math_constants.h>
 #include "common.cuh"

@@ -1,4 +1,4 @@
-// realspace_long.cu -- off-lattice Rosenbluth generation for LONG chains (2048 < N <= 16383), the range of the paper's
+// realspace_long.cu -- off-lattice Rosenbluth generation for LONG chains (400 <= N <= 16383), the range of the paper's
 // real-space "global-memory version" (Table 2: N = 100 ... 10000; Fig. 2b, :296). Same steps R0-R5,
 // the same fp32 arithmetic and therefore the same decisions as realspace.cu, but the chain lives in HBM
 // and the O(s) candidate scan of each step is replaced by a per-chain CELL LIST, so a chain costs O(N k) instead of
