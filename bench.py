@@ -517,8 +517,19 @@ def main():
     ap.add_argument("--paper-tables", action="store_true", help="10^6 chains at every length of the paper's Tables 1-2 instead")
     args = ap.parse_args()
     w = workloads.CONFIGS[args.workload]
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started without torchrun: launch the N ranks ourselves (one process per GPU), never measure 1 GPU as N
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port", str(port),
+                                  os.path.abspath(__file__)] + sys.argv[1:])
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch with torchrun --nproc-per-node {args.gpus}")
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.sweep:
         if rank == 0:

@@ -80,6 +80,9 @@ def load_library() -> C.CDLL:
     L.rosen_realspace_dump.restype = C.c_int
     L.rosen_summary_merge.argtypes = [C.POINTER(rosen_summary), i32, C.POINTER(rosen_summary)]
     L.rosen_summary_merge.restype = C.c_int
+    L.rosen_fit_exponents.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_double), i32, i32,
+                                      C.POINTER(rosen_fit)]
+    L.rosen_fit_exponents.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
     L.rosen_workspace_bytes.restype = C.c_size_t
     L.rosen_workspace_release.argtypes = []
@@ -257,9 +260,6 @@ def rosen_fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> Dict
     """rosen_fit_exponents: nu (Eq. 4) and mu, gamma (Eq. 5-7) by least squares over a length sweep."""
     L = load_library()
     n = len(N)
-    L.rosen_fit_exponents.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int32,
-                                      C.c_int32, C.POINTER(rosen_fit)]
-    L.rosen_fit_exponents.restype = C.c_int
     out = rosen_fit()
     _check(L.rosen_fit_exponents((C.c_int32 * n)(*[int(v) for v in N]), (C.c_double * n)(*[float(v) for v in mean_ree2]),
                                  (C.c_double * n)(*[float(v) for v in ln_mean_W]), n, 1 if use_steps else 0, C.byref(out)))

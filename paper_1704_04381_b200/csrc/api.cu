@@ -52,11 +52,18 @@ int get_scratch(Scratch** out)
     std::lock_guard<std::mutex> lock(g_mutex);
     Scratch& s = g_scratch[dev];
     if (!s.dev) {
-        CK(cudaMalloc(&s.dev, sizeof(Partial) * rosen::kMaxPartials));
-        CK(cudaMalloc(&s.summary_dev, sizeof(rosen_summary)));
-        CK(cudaMalloc(&s.vb_counter, sizeof(uint32_t)));
-        CK(cudaMalloc(&s.lmax, sizeof(double) * (rosen::kMaxPartials + 1)));
-        CK(cudaMallocHost(&s.summary_host, sizeof(rosen_summary)));
+        // all or nothing: a failed allocation must not leave a half-initialised scratch behind for the next call
+        Partial* d = nullptr; rosen_summary* sd = nullptr; uint32_t* vc = nullptr; double* lm = nullptr; rosen_summary* sh = nullptr;
+        cudaError_t e = cudaMalloc(&d, sizeof(Partial) * rosen::kMaxPartials);
+        if (e == cudaSuccess) e = cudaMalloc(&sd, sizeof(rosen_summary));
+        if (e == cudaSuccess) e = cudaMalloc(&vc, sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&lm, sizeof(double) * (rosen::kMaxPartials + 1));
+        if (e == cudaSuccess) e = cudaMallocHost(&sh, sizeof(rosen_summary));
+        if (e != cudaSuccess) {
+            cudaFree(d); cudaFree(sd); cudaFree(vc); cudaFree(lm); if (sh) cudaFreeHost(sh);
+            return fail_cuda(e, "per-device scratch allocation");
+        }
+        s.summary_dev = sd; s.vb_counter = vc; s.lmax = lm; s.summary_host = sh; s.dev = d;
     }
     *out = &s;
     return ROSEN_OK;
@@ -200,9 +207,9 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     Staging st;
     if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
 
-    // largest possible lnW up to N = 512; beyond, the paper's mu = 4.684 (Table 4) keeps exp(lnW - L) inside
-    // fp64 (reading A16)
-    const double ln_shift = std::log(6.0) + (double)(N - 2) * std::log(N <= ROSEN_LATTICE_SCAN_MAX_N ? 5.0 : 4.684);
+    // nominal shift = the largest possible lnW; for N > 512 the call replaces it by the largest lnW it generated, found on
+    // the device before the sums (hp.lmax below, reading A18)
+    const double ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
     if (N >= hash_min_n()) {
         // long chains: per-chain hash map cube -> occupancy bitmap in HBM (lattice_hash.cu)
         rosen::HashParams hp{};
@@ -472,9 +479,10 @@ int rosen_workspace_release(void)
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return ROSEN_OK; }   // nothing was ever allocated
     std::lock_guard<std::mutex> lock(g_mutex);
     Scratch& s = g_scratch[dev];
-    if (s.hash_tables || s.hash_rec) cudaDeviceSynchronize();
+    if (s.hash_tables || s.hash_rec || s.hash_ticket) cudaDeviceSynchronize();
     if (s.hash_tables) { cudaFree(s.hash_tables); s.hash_tables = nullptr; s.hash_tables_bytes = 0; }
     if (s.hash_rec) { cudaFree(s.hash_rec); s.hash_rec = nullptr; s.hash_rec_bytes = 0; }
+    if (s.hash_ticket) { cudaFree(s.hash_ticket); s.hash_ticket = nullptr; }
     return ROSEN_OK;
 }
 int32_t rosen_last_launch_count(void) { return g_launches; }
