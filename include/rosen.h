@@ -138,6 +138,16 @@ ROSEN_API int rosen_realspace_generate_async(int32_t N, uint64_t n_chains, int32
                                    const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
 
 /*
+ * The direction map "rngonsphere" of Alg. 2 line 10 (reading A10) alone, as the real-space
+ * kernels evaluate it: dir_xyz[3 i .. 3 i + 2] = unit vector of the Philox word pair (wz[i], wphi[i]). A component of
+ * step R1 exposed so that parity tests can sweep it exhaustively (all 2^23 polar values; every azimuth octant) against
+ * the oracle and against IEEE arithmetic on the host. wz, wphi, dir_xyz: n, n and 3 n elements, all device pointers
+ * (memory == ROSEN_MEM_DEVICE, enqueue only) or all host pointers (ROSEN_MEM_HOST: staged, synchronous).
+ */
+ROSEN_API int rosen_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* dir_xyz, int32_t memory,
+                                   void* cuda_stream);
+
+/*
  * Conformation dump alone (the store path of PAPER.md:80 / :189, BASELINE config 5): identical to
  * the generate calls with outputs = {conf, lnW} only, provided as named entry points.
  * conf/lnW are DEVICE pointers when memory == ROSEN_MEM_DEVICE, host pointers otherwise.

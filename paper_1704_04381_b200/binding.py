@@ -83,6 +83,8 @@ def load_library() -> C.CDLL:
     L.rosen_fit_exponents.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_double), i32, i32,
                                       C.POINTER(rosen_fit)]
     L.rosen_fit_exponents.restype = C.c_int
+    L.rosen_direction_eval.argtypes = [vp, vp, u64, vp, i32, vp]
+    L.rosen_direction_eval.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
     L.rosen_workspace_bytes.restype = C.c_size_t
     L.rosen_workspace_release.argtypes = []
@@ -264,6 +266,20 @@ def rosen_fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> Dict
     _check(L.rosen_fit_exponents((C.c_int32 * n)(*[int(v) for v in N]), (C.c_double * n)(*[float(v) for v in mean_ree2]),
                                  (C.c_double * n)(*[float(v) for v in ln_mean_W]), n, 1 if use_steps else 0, C.byref(out)))
     return {name: getattr(out, name) for name, _ in out._fields_}
+
+
+def rosen_direction_eval(wz, wphi, stream=None):
+    """rosen_direction_eval: wz, wphi = int32/uint32 CUDA tensors of n Philox words (bit patterns); returns a float32
+    CUDA tensor [n, 3] (enqueue only, on `stream`)."""
+    L = load_library()
+    torch = _torch()
+    n = int(wz.numel())
+    if not (wz.is_cuda and wphi.is_cuda and wz.element_size() == 4 and wphi.element_size() == 4 and wphi.numel() == n
+            and wz.is_contiguous() and wphi.is_contiguous()):
+        raise ValueError("wz, wphi: contiguous 32-bit CUDA tensors of equal length")
+    out = torch.empty((n, 3), dtype=torch.float32, device=wz.device)
+    _check(L.rosen_direction_eval(wz.data_ptr(), wphi.data_ptr(), n, out.data_ptr(), ROSEN_MEM_DEVICE, _stream_ptr(stream)))
+    return out
 
 
 def rosen_workspace_bytes() -> int:

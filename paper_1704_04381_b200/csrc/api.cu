@@ -460,6 +460,33 @@ int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double*
     return ROSEN_OK;
 }
 
+int rosen_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* dir_xyz, int32_t memory, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "direction_eval_kernel";
+    if (!wz || !wphi || !dir_xyz || n == 0 || (memory != ROSEN_MEM_DEVICE && memory != ROSEN_MEM_HOST)) {
+        std::snprintf(g_err, sizeof(g_err), "need wz, wphi, dir_xyz, n >= 1 and a valid memory kind"); return ROSEN_EINVAL;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (memory == ROSEN_MEM_DEVICE) {
+        if (rosen::launch_direction_eval(wz, wphi, n, dir_xyz, stream) < 0) return fail_cuda(cudaGetLastError(), "direction_eval_kernel");
+        ++g_launches;
+        return ROSEN_OK;
+    }
+    uint32_t *dz = nullptr, *dp = nullptr; float* dout = nullptr;
+    cudaError_t e = cudaMallocAsync((void**)&dz, n * 4, stream);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&dp, n * 4, stream);
+    if (e == cudaSuccess) e = cudaMallocAsync((void**)&dout, n * 12, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dz, wz, n * 4, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dp, wphi, n * 4, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess && rosen::launch_direction_eval(dz, dp, n, dout, stream) < 0) e = cudaGetLastError();
+    if (e == cudaSuccess) { ++g_launches; e = cudaMemcpyAsync(dir_xyz, dout, n * 12, cudaMemcpyDeviceToHost, stream); }
+    if (dz) cudaFreeAsync(dz, stream);
+    if (dp) cudaFreeAsync(dp, stream);
+    if (dout) cudaFreeAsync(dout, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    return e == cudaSuccess ? ROSEN_OK : fail_cuda(e, "rosen_direction_eval");
+}
+
 size_t rosen_workspace_bytes(void)
 {
     size_t b = sizeof(Partial) * rosen::kMaxPartials + sizeof(rosen_summary);

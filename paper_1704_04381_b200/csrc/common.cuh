@@ -134,6 +134,8 @@ int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t ch
 int real_long_max_warps(int k, int* warps_out);
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
+// realspace.cu: the direction map of DESIGN.md 3.3 alone, out[3 i ..] = direction(wz[i], wphi[i]) (device pointers)
+int launch_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* out, cudaStream_t stream);
 int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift, const double* ln_shift_dev,
                     void* summary_dev, cudaStream_t stream);   // summary_dev: rosen_summary* in device memory
 

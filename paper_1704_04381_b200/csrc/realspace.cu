@@ -1,13 +1,13 @@
-// realspace.cu -- off-lattice Rosenbluth chain generation for sm_100a (steps R0-R5 of DESIGN.md 2;
-// PAPER.md:185-187 sec. 3.3.3, :202-262 Algorithm 2). A group of G lanes grows one chain: lane =
-// pair of trials (one Philox block), so the trial loop of Alg. 2 line 9 runs across lanes and the
-// free-trial count is a __ballot_sync/__popc. The chain lives in shared memory (SoA fp32).
+// realspace.cu -- off-lattice Rosenbluth chain generation for sm_100a (steps R0-R5 + D1 of DESIGN.md 2;
+// PAPER.md:185-187 sec. 3.3.3, :202-262 Algorithm 2). A group of G lanes grows one chain: a lane owns 2P
+// consecutive trials (P Philox blocks), so the trial loop of Alg. 2 line 9 runs across lanes. The chain lives
+// in shared memory as float4 (x, y, z, -) per monomer, padded with far-away sentinels.
 //
-// Exact pruning of Alg. 2 lines 13-19: a monomer farther than (b + sigma)(1 + 2^-9) from the growth
-// point r_{s-1} cannot be within sigma of any trial (every trial is b(1 +- 1e-6) away from r_{s-1}),
-// so each step first collects the few candidates inside that radius (cooperatively, lanes =
-// monomers) and tests the trials against those only. Decisions are identical to the full scan;
-// the argument with its fp32 error budget is DESIGN.md 5.2.
+// Exact pruning of Alg. 2 lines 13-19: a monomer farther than (b + sigma)(1 + 2^-9) from the growth point
+// r_{s-1} cannot be within sigma of any trial (every trial is b(1 +- 1e-6) away from r_{s-1}), so each step
+// first marks the few candidates inside that radius -- 32 monomers per group and pass, one bit each -- and tests
+// the trials against the marked monomers only. Decisions are identical to the full scan; the argument with its
+// fp32 error budget is DESIGN.md 5.2.
 //
 // All fp32 arithmetic that decides anything is written with explicit __f*_rn intrinsics in the order
 // DESIGN.md 3.3 fixes, so nvcc cannot contract or reorder it.
@@ -22,16 +22,69 @@ namespace rosen {
 
 namespace {
 
+constexpr float kFar = 1.0e18f;   // sentinel coordinate: squared distances ~3e36 stay finite and fail every test
+
 // shared memory carve-up (bytes) -----------------------------------------------------------------
 //   double   ln_tab[256]            ln m, ln_tab[0] = -inf
 //   Partial  scratch[32]
-//   per group: float4 r[Np] (x, y, z, unused); uint16 cand[Np] (byte offsets into r); uint8 mseq[Np]   (Np = N rounded up to 4)
-__host__ __device__ inline int n_pad(int N) { return (N + 3) & ~3; }
-__host__ __device__ inline size_t group_bytes(int N) { return (size_t)n_pad(N) * (16 + 2 + 1) + 4; }
-
-template <int G, int P, bool DIGEST, bool TRAJ>
-__global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const RealParams p)
+//   per group: float4 r[Np] (Np = N rounded up to 32; slots the chain has not reached hold the sentinel);
+//              MSEQ variants: uint8 mseq[Np]
+// The group stride is 16 G (mod 128) bytes for G <= 8, so that the groups of a quarter-warp reading G consecutive
+// monomers each (LDS.128) cover all 32 banks once.
+__host__ __device__ inline int n_pad(int N) { return (N + 31) & ~31; }
+__host__ __device__ inline size_t group_bytes(int N, int G, bool mseq)
 {
+    size_t b = (size_t)n_pad(N) * (mseq ? 17 : 16);
+    const size_t want = (size_t)(16 * G) % 128;
+    b += (want + 128 - b % 128) % 128;
+    return b;
+}
+
+// ---- candidate bits of monomers [j0, j0 + 32) of this lane's group: bit i <=> |r_{j0+i} - h|^2 < prefilter2.
+// cnt = monomers left from j0 (uniform over the warp). Slots beyond the scannable monomers hold the sentinel.
+template <int G>
+__device__ __forceinline__ uint32_t candidate_bits(const float4* R4, int j0, int cnt, int gl, int gshift, uint32_t gmask,
+                                                   float hx, float hy, float hz, float prefilter2)
+{
+    constexpr int Q = 32 / G;                 // monomers per lane and pass
+    if constexpr (G == 32) {
+        const float4 r = R4[j0 + gl];
+        const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
+        return __ballot_sync(0xffffffffu, fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2);
+    } else if constexpr (G >= 8) {
+        uint32_t mask = 0;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            if (G * q >= cnt) break;
+            const float4 r = R4[j0 + G * q + gl];
+            const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
+            const uint32_t b = __ballot_sync(0xffffffffu, fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2);
+            mask |= ((b >> gshift) & gmask) << (G * q);
+        }
+        return mask;
+    } else {
+        uint32_t pm = 0;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            if (G * q >= cnt) break;
+            const float4 r = R4[j0 + G * q + gl];
+            const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
+            if (fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2) pm |= 1u << (G * q);
+        }
+        pm <<= gl;
+#pragma unroll
+        for (int d = 1; d < G; d <<= 1) pm |= __shfl_xor_sync(0xffffffffu, pm, d);
+        return pm;
+    }
+}
+
+// MSEQ: the per-step m sequence is requested (one shared-memory byte per step). The conformation dump needs no
+// variant: the chain is in shared memory anyway and is stored once, after the last step, if p.out.conf is set.
+template <int G, int P, bool DIGEST, bool MSEQ>
+__global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
+{
+    constexpr int T = 2 * P;                                 // trials per lane: t = T * gl + i, i = 0..T-1
+    constexpr uint32_t kFull = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* ln_tab = reinterpret_cast<double*>(smem_raw);
     Partial* scratch = reinterpret_cast<Partial*>(smem_raw + 256 * sizeof(double));
@@ -44,10 +97,8 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
     const uint32_t gmask = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
     const uint32_t below = (1u << gl) - 1u;
     const int group_in_block = threadIdx.x / G;
-    const size_t gsz = (group_bytes(N) + 15) & ~(size_t)15;
-    float4* R4 = reinterpret_cast<float4*>(gbase_ptr + gsz * group_in_block);   // one LDS.128 per monomer
-    uint16_t* cand = reinterpret_cast<uint16_t*>(R4 + Np);
-    uint8_t* mbuf = reinterpret_cast<uint8_t*>(cand + Np);
+    float4* R4 = reinterpret_cast<float4*>(gbase_ptr + group_bytes(N, G, MSEQ) * group_in_block);   // one LDS.128 per monomer
+    uint8_t* mbuf = reinterpret_cast<uint8_t*>(R4 + Np);
 
     for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
     __syncthreads();
@@ -66,14 +117,15 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
 
     for (uint32_t it = 0; it < iters; ++it) {
         const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * gpb + (uint32_t)group_in_block;
-        const bool active = idx < p.n_chains;               // inactive groups compute and discard
+        const bool active = idx < p.n_chains;               // inactive groups of a warp with active ones compute and discard
+        if (!__any_sync(kFull, active)) break;              // idx grows with it: this warp has no chain left in the virtual block
         const uint64_t chain = p.chain_offset + idx;
         const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
 
         // R0
+        for (int i = gl; i < Np; i += G) R4[i] = make_float4(kFar, kFar, kFar, 0.f);
         float hx = 0.f, hy = 0.f, hz = 0.f;
-        if (gl == 0) R4[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-        double lnW = 0.0, Sx = 0.0, Sy = 0.0, Sz = 0.0, S2 = 0.0;
+        double lnW = 0.0;
         bool alive = true;
         uint32_t steps = 0;
         uint64_t dg = 0xCBF29CE484222325ull;
@@ -88,102 +140,113 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
                 usel = (s & 2) ? hi : lo;
             }
 
-            // ---- candidates: monomers j <= s-2 within the conservative radius of r_{s-1}
-            // (two monomers per lane and iteration: independent loads and distance chains hide each other's latency;
-            // the order of the list is irrelevant, overlap is an OR over candidates)
-            int ncand = 0;
-            for (int j0 = 0; j0 < s - 1; j0 += 2 * G) {
-                const int ja = j0 + gl, jb = ja + G;
-                const float4 ra = R4[min(ja, s - 2)], rb = R4[min(jb, s - 2)];
-                const float ax = ra.x - hx, ay = ra.y - hy, az = ra.z - hz;
-                const float bx = rb.x - hx, by = rb.y - hy, bz = rb.z - hz;
-                const bool ina = ja < s - 1 && fmaf(az, az, fmaf(ay, ay, ax * ax)) < p.prefilter2;
-                const bool inb = jb < s - 1 && fmaf(bz, bz, fmaf(by, by, bx * bx)) < p.prefilter2;
-                const uint32_t bita = (__ballot_sync(0xffffffffu, ina) >> gshift) & gmask;
-                const uint32_t bitb = (__ballot_sync(0xffffffffu, inb) >> gshift) & gmask;
-                const int na = __popc(bita);
-                if (ina) cand[ncand + __popc(bita & below)] = (uint16_t)(ja * 16);
-                if (inb) cand[ncand + na + __popc(bitb & below)] = (uint16_t)(jb * 16);
-                ncand += na + __popc(bitb);
-            }
-            __syncwarp();
-
-            // ---- R1 + R2: this lane's trials (P Philox blocks = 2P trials)
-            float tx[P][2], ty[P][2], tz[P][2];
-            bool fr[P][2];
+            // ---- R1: this lane's trials (P Philox blocks = 2P consecutive trials)
+            float tx[T], ty[T], tz[T];
+            bool ov[T];                                      // trial overlaps an earlier monomer (or lies beyond k)
 #pragma unroll
             for (int pp = 0; pp < P; ++pp) {
-                const uint32_t bi = (uint32_t)(gl + G * pp);
+                const uint32_t bi = (uint32_t)(P * gl + pp);
                 uint32_t w[4];
                 philox4x32_10(c_lo, c_hi, (uint32_t)s, 1u + bi, p.key0, p.key1, w);
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     float ux, uy, uz;
                     direction(w[2 * e], w[2 * e + 1], ux, uy, uz);
-                    tx[pp][e] = __fmaf_rn(p.b, ux, hx);
-                    ty[pp][e] = __fmaf_rn(p.b, uy, hy);
-                    tz[pp][e] = __fmaf_rn(p.b, uz, hz);
-                    fr[pp][e] = (int)(2u * bi + e) < k;
+                    tx[2 * pp + e] = __fmaf_rn(p.b, ux, hx);
+                    ty[2 * pp + e] = __fmaf_rn(p.b, uy, hy);
+                    tz[2 * pp + e] = __fmaf_rn(p.b, uz, hz);
+                    ov[2 * pp + e] = (int)(2u * bi + e) >= k;
                 }
-            }
-            for (int c = 0; c < ncand; ++c) {
-                const float4 rj = *reinterpret_cast<const float4*>(reinterpret_cast<const unsigned char*>(R4) + cand[c]);
-                const float xj = rj.x, yj = rj.y, zj = rj.z;
-#pragma unroll
-                for (int pp = 0; pp < P; ++pp)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const float dx = __fsub_rn(xj, tx[pp][e]), dy = __fsub_rn(yj, ty[pp][e]), dz = __fsub_rn(zj, tz[pp][e]);
-                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                        if (d2 < p.sigma2) fr[pp][e] = false;
-                    }
             }
 
-            // ---- m_s and the rank of each free trial in trial order t = 2*(gl + G*pp) + e
-            uint32_t B[P][2];
-            uint32_t m = 0;
+            // ---- R2: monomers j <= s-2 (slots 0..s-2; r_{s-1} itself is stored at the end of this step), 32 per pass:
+            // mark those within the conservative radius of r_{s-1}, then test the trials against the marked ones
+            // (overlap is an OR over monomers: order and batching are irrelevant)
+            for (int j0 = 0; j0 < s - 1; j0 += 32) {
+                uint32_t mask = candidate_bits<G>(R4, j0, s - 1 - j0, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
+                while (mask) {
+                    const int bpos = 31 - __clz(mask);
+                    mask ^= 1u << bpos;
+                    const float4 rj = R4[j0 + bpos];
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    B[pp][e] = (__ballot_sync(0xffffffffu, fr[pp][e]) >> gshift) & gmask;
-                    m += __popc(B[pp][e]);
+                    for (int i = 0; i < T; ++i) {
+                        const float dx = __fsub_rn(rj.x, tx[i]), dy = __fsub_rn(rj.y, ty[i]), dz = __fsub_rn(rj.z, tz[i]);
+                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                        ov[i] = ov[i] || d2 < p.sigma2;
+                    }
                 }
+            }
+
+            // ---- m_s and the number of free trials of lower lanes (trial order = lane order, then i)
+            uint32_t f = 0;
+#pragma unroll
+            for (int i = 0; i < T; ++i) f |= ov[i] ? 0u : 1u << i;
+            const uint32_t c = __popc(f);
+            uint32_t m, excl;
+            if constexpr (G == 1) {
+                m = c; excl = 0;
+            } else if constexpr (G <= 4) {
+                uint32_t V = c << (8 * gl);                  // one byte per lane (c <= 8)
+#pragma unroll
+                for (int d = 1; d < G; d <<= 1) V |= __shfl_xor_sync(kFull, V, d);
+                const uint32_t cum = V * 0x01010101u;        // byte j = c_0 + ... + c_j (no carries: total <= 32)
+                m = cum >> 24;
+                excl = ((cum << 8) >> (8 * gl)) & 0xFFu;
+            } else {
+                m = 0; excl = 0;
+#pragma unroll
+                for (int i = 0; i < T; ++i) {
+                    const uint32_t B = (__ballot_sync(kFull, (f >> i) & 1u) >> gshift) & gmask;
+                    m += __popc(B); excl += __popc(B & below);
+                }
+            }
 
             // ---- R3
             steps += alive ? 1u : 0u;
             lnW += ln_tab[m];
-            if (TRAJ) { if (gl == 0 && p.out.m_seq) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
+            if (MSEQ) { if (gl == 0) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
 
-            // ---- R4: the sel-th free trial
+            // ---- R4: the sel-th free trial; it is this lane's if excl <= sel < excl + c, namely the (sel - excl)-th set bit of f
             const uint32_t sel = __umulhi(usel, m);
-            uint32_t base = 0;
-            bool hit = false;
-            float px = hx, py = hy, pz = hz;
-            uint32_t tsel = 0;
+            const uint32_t rk = sel - excl;
+            const bool hit = rk < c;
+            uint32_t g2 = f;
 #pragma unroll
-            for (int pp = 0; pp < P; ++pp) {
-                const uint32_t r0 = base + __popc(B[pp][0] & below) + __popc(B[pp][1] & below);
-                const uint32_t r1 = r0 + (fr[pp][0] ? 1u : 0u);
-                if (fr[pp][0] && r0 == sel) { hit = true; px = tx[pp][0]; py = ty[pp][0]; pz = tz[pp][0]; tsel = 2u * (gl + G * pp); }
-                if (fr[pp][1] && r1 == sel) { hit = true; px = tx[pp][1]; py = ty[pp][1]; pz = tz[pp][1]; tsel = 2u * (gl + G * pp) + 1u; }
-                base += __popc(B[pp][0]) + __popc(B[pp][1]);
+            for (int i = 0; i < T - 1; ++i) g2 = (rk > (uint32_t)i) ? (g2 & (g2 - 1u)) : g2;
+            const int li = __ffs(g2) - 1;
+            float px = tx[0], py = ty[0], pz = tz[0];
+#pragma unroll
+            for (int i = 1; i < T; ++i)
+                if (li == i) { px = tx[i]; py = ty[i]; pz = tz[i]; }
+            uint32_t tsel = (uint32_t)(T * gl + li);
+            if constexpr (G > 1) {
+                const uint32_t hb = (__ballot_sync(kFull, hit) >> gshift) & gmask;
+                const int src = gshift + (hb ? __ffs(hb) - 1 : 0);
+                px = __shfl_sync(kFull, px, src); py = __shfl_sync(kFull, py, src); pz = __shfl_sync(kFull, pz, src);
+                if (DIGEST) tsel = __shfl_sync(kFull, tsel, src);
             }
-            const uint32_t hb = (__ballot_sync(0xffffffffu, hit) >> gshift) & gmask;
-            const int src = gshift + (hb ? __ffs(hb) - 1 : 0);
-            px = __shfl_sync(0xffffffffu, px, src); py = __shfl_sync(0xffffffffu, py, src);
-            pz = __shfl_sync(0xffffffffu, pz, src); tsel = __shfl_sync(0xffffffffu, tsel, src);
             if (DIGEST) { if (alive) dg = digest_fold(dg, m, m ? tsel : 0xFFu); }
+            if (gl == 0) R4[s - 1] = make_float4(hx, hy, hz, 0.f);      // r_{s-1} becomes scannable from step s+1 on
             alive = alive && (m != 0u);
             if (m != 0u) { hx = px; hy = py; hz = pz; }
-            if (gl == 0) R4[s] = make_float4(hx, hy, hz, 0.f);
-
-            // ---- R5 running sums (fp64)
-            Sx += (double)hx; Sy += (double)hy; Sz += (double)hz;
-            S2 += (double)hx * (double)hx + (double)hy * (double)hy + (double)hz * (double)hz;
             __syncwarp();
         }
+        if (gl == 0) R4[N - 1] = make_float4(hx, hy, hz, 0.f);
+        __syncwarp();
 
+        // ---- R5: fp64 sums over the finished chain, the group's lanes in parallel, then a butterfly (every lane
+        // of the group ends with the same bits: a + b == b + a)
+        double Sx = 0.0, Sy = 0.0, Sz = 0.0, S2 = 0.0;
+        for (int i = gl; i < N; i += G) {
+            const float4 r = R4[i];
+            const double x = (double)r.x, y = (double)r.y, z = (double)r.z;
+            Sx += x; Sy += y; Sz += z; S2 += x * x + y * y + z * z;
+        }
+#pragma unroll
+        for (int d = 1; d < G; d <<= 1) {
+            Sx += __shfl_xor_sync(kFull, Sx, d); Sy += __shfl_xor_sync(kFull, Sy, d);
+            Sz += __shfl_xor_sync(kFull, Sz, d); S2 += __shfl_xor_sync(kFull, S2, d);
+        }
         double ree2 = 0.0, rg2 = 0.0;
         if (alive) {
             ree2 = (double)hx * (double)hx + (double)hy * (double)hy + (double)hz * (double)hz;
@@ -202,21 +265,34 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
             if (p.out.rg2) p.out.rg2[idx] = rg2;
             if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
         }
-        if (TRAJ && active) {
-            // D1: the group streams its chain out of shared memory, interleaving SoA -> [N][3]
+        // ---- D1: the group streams its chain out of shared memory, float4 (x, y, z, -) -> [N][3], zeros from the
+        // death step on. Rows are 12 N bytes: 16-byte aligned when N is a multiple of 4, then consecutive lanes store
+        // consecutive 16-byte pieces (G = 32: 512 contiguous bytes per instruction); otherwise 4-byte stores.
+        if (p.out.conf != nullptr && active) {
             const int placed = alive ? N : (int)steps;
-            if (p.out.conf) {
-                float* c = reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3;
+            const float* Rf = reinterpret_cast<const float*>(R4);
+            float* crow = reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3;
+            if ((N & 3) == 0) {
+                float4* c4 = reinterpret_cast<float4*>(crow);
+                for (int v = gl; v < 3 * (N >> 2); v += G) {
+                    float o[4];
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) {
+                        const uint32_t e = 4u * (uint32_t)v + cc, i = (e * 43691u) >> 17;       // e / 3 for e < 98304
+                        o[cc] = (int)i < placed ? Rf[e + i] : 0.0f;                                // word 4 i + (e - 3 i)
+                    }
+                    c4[v] = make_float4(o[0], o[1], o[2], o[3]);
+                }
+            } else {
                 for (int e = gl; e < 3 * N; e += G) {
-                    const int i = e / 3, a = e - 3 * i;
-                    const float v = reinterpret_cast<const float*>(R4)[4 * i + a];
-                    c[e] = i < placed ? v : 0.0f;
+                    const uint32_t i = ((uint32_t)e * 43691u) >> 17;
+                    crow[e] = (int)i < placed ? Rf[e + i] : 0.0f;
                 }
             }
-            if (p.out.m_seq) {
-                uint8_t* mr = p.out.m_seq + idx * (uint64_t)(N - 1);
-                for (int e = gl; e < N - 1; e += G) mr[e] = mbuf[e];
-            }
+        }
+        if (MSEQ && active) {
+            uint8_t* mr = p.out.m_seq + idx * (uint64_t)(N - 1);
+            for (int e = gl; e < N - 1; e += G) mr[e] = mbuf[e];
         }
         __syncwarp();
     }
@@ -225,7 +301,17 @@ __global__ void __launch_bounds__(256, TRAJ ? 3 : 0) realspace_kernel(const Real
     }
 }
 
-template <int G, int P, bool DIGEST, bool TRAJ>
+// threads per block: a function of (N, G) only -- it fixes the reduction tree, so it must not depend on the output variant
+int block_threads(int N, int G)
+{
+    const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
+    const size_t gsz = group_bytes(N, G, true);
+    int threads = 256;
+    while (threads > 32 && fixed + gsz * (threads / G) > (size_t)(74 * 1024 + 512)) threads >>= 1;   // three blocks per SM
+    return threads;
+}
+
+template <int G, int P, bool DIGEST, bool MSEQ>
 int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
 {
     int dev = 0, n_sm = 0, smem_max = 0;
@@ -233,12 +319,10 @@ int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
-    const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
-    int threads = 256;
-    while (threads > 32 && fixed + gsz * (threads / G) > (size_t)(100 * 1024)) threads >>= 1;
-    const size_t smem = fixed + gsz * (threads / G);
+    const int threads = block_threads(p.N, G);
+    const size_t smem = fixed + group_bytes(p.N, G, MSEQ) * (threads / G);
     if (smem > (size_t)smem_max) return -2;
-    auto kern = realspace_kernel<G, P, DIGEST, TRAJ>;
+    auto kern = realspace_kernel<G, P, DIGEST, MSEQ>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
@@ -255,12 +339,30 @@ template <int G, int P>
 int launch_gp(const RealParams& p, cudaStream_t stream, int* grid_out)
 {
     const bool digest = p.out.digest != nullptr;
-    const bool traj = p.out.m_seq != nullptr || p.out.conf != nullptr;
-    if (traj) return digest ? launch_one<G, P, true, true>(p, stream, grid_out) : launch_one<G, P, false, true>(p, stream, grid_out);
+    const bool mseq = p.out.m_seq != nullptr;
+    if (mseq) return digest ? launch_one<G, P, true, true>(p, stream, grid_out) : launch_one<G, P, false, true>(p, stream, grid_out);
     return digest ? launch_one<G, P, true, false>(p, stream, grid_out) : launch_one<G, P, false, false>(p, stream, grid_out);
 }
 
+// direction map alone (test entry rosen_direction_eval): out[3 i ..] = direction(wz[i], wphi[i])
+__global__ void direction_eval_kernel(const uint32_t* __restrict__ wz, const uint32_t* __restrict__ wphi, uint64_t n,
+                                      float* __restrict__ out)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        float ux, uy, uz;
+        direction(wz[i], wphi[i], ux, uy, uz);
+        out[3 * i] = ux; out[3 * i + 1] = uy; out[3 * i + 2] = uz;
+    }
+}
+
 }  // namespace
+
+int launch_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* out, cudaStream_t stream)
+{
+    const uint64_t blocks = (n + 255) / 256;
+    direction_eval_kernel<<<(int)(blocks < 4096 ? blocks : 4096), 256, 0, stream>>>(wz, wphi, n, out);
+    return cudaGetLastError() == cudaSuccess ? 1 : -3;
+}
 
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out)
 {
@@ -268,7 +370,7 @@ int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kern
     // Long chains: a warp holds 32/G chains of group_bytes(N) each; widen the group (idle lanes own trials >= k)
     // until one warp's chains fit 24 KB, so that a block of >= 4 warps fits shared memory (N = 2048: one chain per warp, 2 warps per block).
     {
-        const size_t gsz = (group_bytes(p.N) + 15) & ~(size_t)15;
+        const size_t gsz = (size_t)n_pad(p.N) * 17;
         int g_mem = 1;
         while (g_mem < 32 && (32 / g_mem) * gsz > (size_t)(24 * 1024)) g_mem *= 2;
         if (g_mem > 4 && blocks < g_mem) blocks = g_mem;      // selects <G = g_mem, P = 1> below (g_mem = 8 -> G = 16)

@@ -186,3 +186,49 @@ def test_config3_full_size_sampled(R):
         assert math.isclose(re[i], oi.ree2[0], rel_tol=1e-12, abs_tol=1e-12)
     assert flips == 0
     assert 0.01 < s["attrition"] < 0.03 and 180 < s["mean_ree2"] < 230     # 1.7 %, ~201
+
+
+def test_direction_map_vs_oracle(R):
+    """R1's direction map alone (rosen_direction_eval) against the oracle's, bit for bit: 200 000 random word pairs and
+    every octant edge (the two sides execute the same IEEE operations)."""
+    import torch
+    rng = np.random.default_rng(777)
+    wz = rng.integers(0, 2 ** 32, size=200000, dtype=np.uint64)
+    wphi = rng.integers(0, 2 ** 32, size=200000, dtype=np.uint64)
+    edge_phi = [(((o << 21) | f) << 8) | low for o in range(8) for f in (0, 1, 0x0FFFFF, 0x100000, 0x1FFFFE, 0x1FFFFF)
+                for low in (0, 0xFF)]
+    edge_z = [0, 0x1FF, 0x200, 0x80000000, 0x7FFFFFFF, 0xFFFFFE00, 0xFFFFFFFF]
+    ez, ep = np.meshgrid(np.array(edge_z, dtype=np.uint64), np.array(edge_phi, dtype=np.uint64))
+    wz = np.concatenate([wz, ez.ravel()]); wphi = np.concatenate([wphi, ep.ravel()])
+    tz = torch.from_numpy(wz.astype(np.uint32).view(np.int32)).cuda()
+    tp = torch.from_numpy(wphi.astype(np.uint32).view(np.int32)).cuda()
+    got = R.rosen_direction_eval(tz, tp).cpu().numpy()
+    want = np.stack([oracle.direction(int(a), int(b)) for a, b in zip(wz, wphi)])
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+
+
+def test_direction_map_exhaustive_z(R):
+    """All 2^23 polar values the map can produce, at one azimuth per octant, against IEEE arithmetic done on the host:
+    z = (2q+1) 2^-23 - 1 exactly; a = fl32(1 - z^2) (exact in fp64, rounded once = the fma); rho = IEEE sqrt in fp32;
+    u = (fl32(rho c), fl32(rho s), z) with (c, s) the oracle's azimuth factors at z = 2^-23... (rho = 1 there up to one
+    rounding, see below). Pins the kernel's own square-root sequence (csrc/direction.cuh sqrt_rn_unit) for every argument."""
+    import torch
+    q = np.arange(1 << 23, dtype=np.uint64)
+    wz = (q << 9).astype(np.uint32)
+    z64 = (2.0 * q.astype(np.float64) + 1.0) * 2.0 ** -23 - 1.0                 # exact
+    a32 = (1.0 - z64 * z64).astype(np.float32)                                   # 1 - z^2 exact in fp64, one rounding
+    rho = np.sqrt(a32)                                                           # IEEE correctly rounded fp32 sqrt
+    assert rho.dtype == np.float32 and a32.min() > 2.0 ** -23
+    tz = torch.from_numpy(wz.view(np.int32)).cuda()
+    for oct_ in range(8):
+        wphi = ((oct_ << 21) | 0x0ABCDE) << 8
+        # azimuth factors (c, s): the oracle at the equator-most z (q = 2^22: z = 2^-23, a = fl32(1 - 2^-46) = 1, rho = 1)
+        cs = oracle.direction(1 << 31, wphi)
+        assert cs[2] == np.float32(2.0 ** -23)
+        tp = torch.full((1 << 23,), wphi if wphi < 2 ** 31 else wphi - 2 ** 32, dtype=torch.int32, device="cuda")
+        got = R.rosen_direction_eval(tz, tp).cpu().numpy()
+        ux = (rho.astype(np.float64) * float(cs[0])).astype(np.float32)          # 24 x 24 bit product exact in fp64
+        uy = (rho.astype(np.float64) * float(cs[1])).astype(np.float32)
+        assert np.array_equal(got[:, 2], z64.astype(np.float32))
+        assert np.array_equal(got[:, 0].view(np.uint32), ux.view(np.uint32))
+        assert np.array_equal(got[:, 1].view(np.uint32), uy.view(np.uint32))
