@@ -40,37 +40,63 @@ __host__ __device__ inline size_t group_bytes(int N, int G, bool mseq)
     return b;
 }
 
+__device__ __forceinline__ uint32_t bfind(uint32_t x)     // index of the most significant set bit (FLO.U32)
+{
+    uint32_t r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
+
+// t = |r - h|^2 - prefilter2 in one FFMA chain: negative (sign bit set) iff the monomer is inside the conservative radius
+// (an exact zero rounds to +0). Its few-ulp rounding is covered by the radius margin like that of the plain sum.
+__device__ __forceinline__ uint32_t inside_bits(const float4 r, float hx, float hy, float hz, float prefilter2)
+{
+    const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
+    return __float_as_uint(fmaf(az, az, fmaf(ay, ay, fmaf(ax, ax, -prefilter2))));
+}
+
 // ---- candidate bits of monomers [j0, j0 + 32) of this lane's group: bit i <=> |r_{j0+i} - h|^2 < prefilter2.
-// cnt = monomers left from j0 (uniform over the warp). Slots beyond the scannable monomers hold the sentinel.
+// base = R4 + j0; cnt = monomers left from j0 (>= 1, uniform over the warp). Slots beyond the scannable monomers hold the
+// sentinel. Lane gl looks at slots G q + gl, q = 0 .. min(Q, ceil(cnt / G)) - 1.
 template <int G>
-__device__ __forceinline__ uint32_t candidate_bits(const float4* R4, int j0, int cnt, int gl, int gshift, uint32_t gmask,
-                                                   float hx, float hy, float hz, float prefilter2)
+__device__ __forceinline__ uint32_t candidate_bits(const float4* base, int cnt, int gl, int gshift, uint32_t gmask,
+                                                   float hx, float hy, float hz, float pf)
 {
     constexpr int Q = 32 / G;                 // monomers per lane and pass
     if constexpr (G == 32) {
-        const float4 r = R4[j0 + gl];
-        const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
-        return __ballot_sync(0xffffffffu, fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2);
+        return __ballot_sync(0xffffffffu, (int32_t)inside_bits(base[gl], hx, hy, hz, pf) < 0);
     } else if constexpr (G >= 8) {
         uint32_t mask = 0;
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
             if (G * q >= cnt) break;
-            const float4 r = R4[j0 + G * q + gl];
-            const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
-            const uint32_t b = __ballot_sync(0xffffffffu, fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2);
+            const uint32_t b = __ballot_sync(0xffffffffu, (int32_t)inside_bits(base[G * q + gl], hx, hy, hz, pf) < 0);
             mask |= ((b >> gshift) & gmask) << (G * q);
         }
         return mask;
     } else {
         uint32_t pm = 0;
+        const float4* lb = base + gl;
+#define ROSEN_PF(q) pm |= (inside_bits(lb[G * (q)], hx, hy, hz, pf) >> (31 - G * (q))) & (1u << (G * (q)));
+        if constexpr (G == 4) {               // one computed jump per pass instead of a test per monomer
+            switch ((cnt + 3) >> 2) {
+                default: ROSEN_PF(7)
+                case 7: ROSEN_PF(6)
+                case 6: ROSEN_PF(5)
+                case 5: ROSEN_PF(4)
+                case 4: ROSEN_PF(3)
+                case 3: ROSEN_PF(2)
+                case 2: ROSEN_PF(1)
+                case 1: ROSEN_PF(0)
+            }
+        } else {
 #pragma unroll
-        for (int q = 0; q < Q; ++q) {
-            if (G * q >= cnt) break;
-            const float4 r = R4[j0 + G * q + gl];
-            const float ax = r.x - hx, ay = r.y - hy, az = r.z - hz;
-            if (fmaf(az, az, fmaf(ay, ay, ax * ax)) < prefilter2) pm |= 1u << (G * q);
+            for (int q = 0; q < Q; ++q) {
+                if (G * q >= cnt) break;
+                ROSEN_PF(q)
+            }
         }
+#undef ROSEN_PF
         pm <<= gl;
 #pragma unroll
         for (int d = 1; d < G; d <<= 1) pm |= __shfl_xor_sync(0xffffffffu, pm, d);
@@ -134,15 +160,19 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
         __syncwarp();
 
         for (int s = 1; s < N; ++s) {
-            if ((s & 3) == 0 || s == 1) philox4x32_10(c_lo, c_hi, (uint32_t)(s >> 2), 0u, p.key0, p.key1, selw);
+            // selection word u_s = word s & 3 of block s >> 2: lane gl draws the blocks with (s >> 2) = gl (mod G), once per
+            // 4 G steps, and the owner's word is broadcast (one Philox block per 4 steps and GROUP instead of per lane)
+            if (s == 1 || (s & (4 * G - 1)) == 0)
+                philox4x32_10(c_lo, c_hi, (uint32_t)(((s >> 2) & ~(G - 1)) + gl), 0u, p.key0, p.key1, selw);
             {   // word s & 3 without a dynamically indexed (local-memory) array
                 const uint32_t lo = (s & 1) ? selw[1] : selw[0], hi = (s & 1) ? selw[3] : selw[2];
                 usel = (s & 2) ? hi : lo;
+                if constexpr (G > 1) usel = __shfl_sync(kFull, usel, gshift + ((s >> 2) & (G - 1)));
             }
 
             // ---- R1: this lane's trials (P Philox blocks = 2P consecutive trials)
             float tx[T], ty[T], tz[T];
-            bool ov[T];                                      // trial overlaps an earlier monomer (or lies beyond k)
+            float near2[T];                                  // smallest spec'd d2 to an earlier monomer so far (-1: trial index >= k)
 #pragma unroll
             for (int pp = 0; pp < P; ++pp) {
                 const uint32_t bi = (uint32_t)(P * gl + pp);
@@ -155,7 +185,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
                     tx[2 * pp + e] = __fmaf_rn(p.b, ux, hx);
                     ty[2 * pp + e] = __fmaf_rn(p.b, uy, hy);
                     tz[2 * pp + e] = __fmaf_rn(p.b, uz, hz);
-                    ov[2 * pp + e] = (int)(2u * bi + e) >= k;
+                    near2[2 * pp + e] = (int)(2u * bi + e) < k ? CUDART_MAX_NORMAL_F : -1.0f;
                 }
             }
 
@@ -163,16 +193,17 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             // mark those within the conservative radius of r_{s-1}, then test the trials against the marked ones
             // (overlap is an OR over monomers: order and batching are irrelevant)
             for (int j0 = 0; j0 < s - 1; j0 += 32) {
-                uint32_t mask = candidate_bits<G>(R4, j0, s - 1 - j0, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
+                const float4* pb = R4 + j0;
+                uint32_t mask = candidate_bits<G>(pb, s - 1 - j0, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
                 while (mask) {
-                    const int bpos = 31 - __clz(mask);
+                    const uint32_t bpos = bfind(mask);
                     mask ^= 1u << bpos;
-                    const float4 rj = R4[j0 + bpos];
+                    const float4 rj = pb[bpos];
 #pragma unroll
                     for (int i = 0; i < T; ++i) {
                         const float dx = __fsub_rn(rj.x, tx[i]), dy = __fsub_rn(rj.y, ty[i]), dz = __fsub_rn(rj.z, tz[i]);
                         const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                        ov[i] = ov[i] || d2 < p.sigma2;
+                        near2[i] = fminf(near2[i], d2);      // overlap iff some d2 < sigma2 iff the smallest is
                     }
                 }
             }
@@ -180,7 +211,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             // ---- m_s and the number of free trials of lower lanes (trial order = lane order, then i)
             uint32_t f = 0;
 #pragma unroll
-            for (int i = 0; i < T; ++i) f |= ov[i] ? 0u : 1u << i;
+            for (int i = 0; i < T; ++i) f |= near2[i] < p.sigma2 ? 0u : 1u << i;
             const uint32_t c = __popc(f);
             uint32_t m, excl;
             if constexpr (G == 1) {
