@@ -56,6 +56,20 @@ def lib() -> C.CDLL:
         L.oracle_saw_enumerate.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                            C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         L.oracle_saw_enumerate.restype = C.c_int
+        L.oracle_model_table.argtypes = [C.c_double, C.POINTER(C.c_uint64)]
+        L.oracle_model_table.restype = None
+        L.oracle_lattice_model_step.argtypes = [C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.POINTER(C.c_uint64),
+                                                C.POINTER(C.c_uint64)]
+        L.oracle_lattice_model_step.restype = C.c_int32
+        L.oracle_lattice_model_generate.argtypes = [C.c_int32, C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32, C.c_double,
+                                                    C.POINTER(_Outputs), C.POINTER(_Summary)]
+        L.oracle_lattice_model_generate.restype = C.c_int
+        L.oracle_realspace_model_generate.argtypes = [C.c_int32, C.c_uint64, C.c_int32, C.c_float, C.c_float, C.c_float,
+                                                      C.c_double, C.c_uint64, C.c_uint64, C.POINTER(_Outputs),
+                                                      C.POINTER(_Summary)]
+        L.oracle_realspace_model_generate.restype = C.c_int
+        L.oracle_saw_enumerate_model.argtypes = [C.c_int32, C.c_int32, C.c_double, C.POINTER(C.c_double)]
+        L.oracle_saw_enumerate_model.restype = C.c_int
         _LIB = L
     return _LIB
 
@@ -112,6 +126,53 @@ def realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: float, si
     if rc != 0:
         raise ValueError(f"oracle_realspace_generate: invalid arguments (rc={rc})")
     return Result(summary=_summary_dict(s), **arrs)
+
+
+def lattice_model_generate(N: int, n_chains: int, seed: int, z: int = 6, beta_eps: float = 0.0, chain_offset: int = 0,
+                           outputs=ALL) -> Result:
+    """Lattice chains with the z = 6 / 26 trial set and contact energy -eps per non-bonded neighbour pair
+    (Boltzmann-weighted trials)."""
+    arrs, out = _alloc(n_chains, N, np.int32, set(outputs))
+    s = _Summary()
+    rc = lib().oracle_lattice_model_generate(N, n_chains, seed, chain_offset, z, beta_eps, C.byref(out), C.byref(s))
+    if rc != 0:
+        raise ValueError(f"oracle_lattice_model_generate: invalid arguments (rc={rc})")
+    return Result(summary=_summary_dict(s), **arrs)
+
+
+def realspace_model_generate(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, lam: float,
+                             beta_eps: float, seed: int, chain_offset: int = 0, outputs=ALL) -> Result:
+    """Real-space chains with a square-well attraction of range lam * sigma and depth eps."""
+    arrs, out = _alloc(n_chains, N, np.float32, set(outputs))
+    s = _Summary()
+    rc = lib().oracle_realspace_model_generate(N, n_chains, k_trials, bond_len, sigma, lam, beta_eps, seed, chain_offset,
+                                               C.byref(out), C.byref(s))
+    if rc != 0:
+        raise ValueError(f"oracle_realspace_model_generate: invalid arguments (rc={rc})")
+    return Result(summary=_summary_dict(s), **arrs)
+
+
+def model_table(beta_eps: float) -> list:
+    q = (C.c_uint64 * 32)()
+    lib().oracle_model_table(beta_eps, q)
+    return [int(v) for v in q]
+
+
+def lattice_model_step(r: np.ndarray, z: int, beta_eps: float) -> list:
+    """Per-trial fixed-point weights (0 = occupied) for the next monomer of walk r [s][3]."""
+    r = np.ascontiguousarray(r, dtype=np.int32)
+    q = (C.c_uint64 * 32)(*model_table(beta_eps))
+    w = (C.c_uint64 * 26)()
+    lib().oracle_lattice_model_step(r.ctypes.data_as(C.POINTER(C.c_int32)), r.shape[0], z, q, w)
+    return [int(w[d]) for d in range(z)]
+
+
+def saw_enumerate_model(n: int, z: int, beta_eps: float) -> dict:
+    out = (C.c_double * 5)()
+    rc = lib().oracle_saw_enumerate_model(n, z, beta_eps, out)
+    if rc != 0:
+        raise RuntimeError(f"oracle_saw_enumerate_model rc={rc}")
+    return dict(zip(("count", "sum_boltz", "sum_boltz_ree2", "sum_quant", "sum_prob"), [float(v) for v in out]))
 
 
 def philox4x32_10(ctr, key) -> tuple:

@@ -383,4 +383,241 @@ int oracle_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_trials, fl
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Other trial sets and Boltzmann-weighted trials (readings A19-A21).
+//
+//   * z = 26: "randomly chosen within all z = 26 possible lattice space" (sec. 3.3.2): the trial sites
+//     are the 26 sites (dx,dy,dz) in {-1,0,1}^3 \ {0} around r_{s-1}, in the order i = (dx+1) + 3(dy+1) + 9(dz+1)
+//     (i = 13, the centre, skipped); self-avoidance is site exclusion only.
+//   * Boltzmann weights (Eq. 1-2: configurations enter with exp[-beta U] / P_s): U = -eps per
+//     non-bonded contact (lattice: an earlier monomer on one of the z neighbour sites of the new monomer; real space:
+//     an earlier monomer closer than lambda sigma), so a free trial t that would make c_t contacts carries the factor
+//     q^c_t, q = exp(beta eps); the step's Rosenbluth factor is W_s = sum_t q^c_t and trial t is taken with
+//     probability q^c_t / W_s. beta eps = 0 gives back W_s = m_s and the uniform choice of Alg. 1 / Alg. 2.
+//   * The factors are FIXED-POINT integers Q[c] = round(q^c 2^16) (q^c by repeated fp64 multiplication), so W_s and
+//     the cumulative sums of the choice are exact integers, independent of summation order; the choice is the first
+//     trial, in trial order, whose cumulative sum exceeds floor(u_s W_s / 2^32). lnW += log(W_s 2^-16) in fp64.
+// ---------------------------------------------------------------------------------------------
+void oracle_model_table(double beta_eps, uint64_t Q[32])
+{
+    const double q = std::exp(beta_eps);
+    double p = 1.0;
+    for (int c = 0; c < 32; ++c) { Q[c] = (uint64_t)std::llround(p * 65536.0); p *= q; }
+}
+
+static void model_dir(int32_t z, int32_t d, int32_t e[3])
+{
+    if (z == 6) { e[0] = E[d][0]; e[1] = E[d][1]; e[2] = E[d][2]; return; }
+    const int32_t i = d < 13 ? d : d + 1;
+    e[0] = i % 3 - 1; e[1] = (i / 3) % 3 - 1; e[2] = i / 9 - 1;
+}
+
+static bool model_neighbours(int32_t z, const int32_t a[3], const int32_t b[3])
+{
+    const int32_t dx = std::abs(a[0] - b[0]), dy = std::abs(a[1] - b[1]), dz = std::abs(a[2] - b[2]);
+    if (dx + dy + dz == 0) return false;
+    return z == 6 ? dx + dy + dz == 1 : (dx <= 1 && dy <= 1 && dz <= 1);
+}
+
+// One growth step of the lattice model: r = s placed monomers [s][3]; for every trial d (order above) w[d] = 0 if the
+// site r[s-1] + e_d is occupied by some r[j], j <= s-2, else Q[c_d] with c_d = number of j <= s-2 whose site is a
+// z-neighbour of the trial site (the bonded predecessor r[s-1] is not counted). Returns m = number of free trials.
+int32_t oracle_lattice_model_step(const int32_t* r, int32_t s, int32_t z, const uint64_t Q[32], uint64_t w[26])
+{
+    int32_t m = 0;
+    for (int32_t d = 0; d < z; ++d) {
+        int32_t e[3], t[3];
+        model_dir(z, d, e);
+        for (int a = 0; a < 3; ++a) t[a] = r[3 * (s - 1) + a] + e[a];
+        bool overlap = false;
+        int32_t c = 0;
+        for (int32_t j = 0; j < s - 1; ++j) {
+            if (r[3*j] == t[0] && r[3*j+1] == t[1] && r[3*j+2] == t[2]) overlap = true;
+            if (model_neighbours(z, &r[3*j], t)) ++c;
+        }
+        w[d] = overlap ? 0 : Q[c];
+        if (!overlap) ++m;
+    }
+    return m;
+}
+
+// floor(u W / 2^32) for a 32-bit u and W < 2^63, without a 128-bit product
+static uint64_t scaled_target(uint32_t u, uint64_t W)
+{
+    return (W >> 32) * (uint64_t)u + (((W & 0xFFFFFFFFull) * (uint64_t)u) >> 32);
+}
+
+int oracle_lattice_model_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, int32_t z,
+                                  double beta_eps, const oracle_outputs* out, oracle_summary* summary)
+{
+    if (N < 2 || n_chains == 0 || (z != 6 && z != 26) || !(beta_eps >= 0.0) || !(beta_eps <= 0.85)) return -1;
+    uint64_t Q[32];
+    oracle_model_table(beta_eps, Q);
+    std::vector<int32_t> r((size_t)N * 3);
+    std::vector<ChainResult> res;
+    res.reserve(n_chains);
+    uint64_t n_steps = 0, dxor = 0, dsum = 0;
+
+    for (uint64_t i = 0; i < n_chains; ++i) {
+        const uint64_t chain = chain_offset + i;
+        std::fill(r.begin(), r.end(), 0);
+        double lnW = 0.0;
+        bool alive = true;
+        uint64_t h = digest_init();
+        uint8_t* mrow = (out && out->m_seq) ? out->m_seq + i * (size_t)(N - 1) : nullptr;
+        if (mrow) std::memset(mrow, 0, (size_t)(N - 1));
+
+        for (int32_t s = 1; s <= N - 1; ++s) {
+            uint64_t w[26];
+            const int32_t m = oracle_lattice_model_step(r.data(), s, z, Q, w);
+            ++n_steps;
+            if (mrow) mrow[s - 1] = (uint8_t)m;
+            if (m == 0) {
+                alive = false; h = digest_fold(h, 0, 0xFF);
+                for (int32_t q = s; q < N; ++q) r[3*q] = r[3*q+1] = r[3*q+2] = 0;
+                break;
+            }
+            uint64_t W = 0;
+            for (int32_t d = 0; d < z; ++d) W += w[d];
+            lnW += std::log((double)W * 0x1p-16);                          // W_s = sum_t q^c_t
+            const uint64_t target = scaled_target(selection_word(seed, chain, (uint32_t)s), W);
+            int32_t d = 0;
+            uint64_t cum = w[0];
+            while (cum <= target) cum += w[++d];                         // first trial whose cumulative sum exceeds the target
+            int32_t e[3];
+            model_dir(z, d, e);
+            for (int a = 0; a < 3; ++a) r[3*s+a] = r[3*(s-1)+a] + e[a];
+            h = digest_fold(h, (uint32_t)m, (uint32_t)d);
+        }
+
+        double ree2 = 0.0, rg2 = 0.0;
+        if (alive) {
+            int64_t sx = 0, sy = 0, sz = 0, s2 = 0;
+            for (int32_t q = 0; q < N; ++q) {
+                const int64_t x = r[3*q], y = r[3*q+1], zz = r[3*q+2];
+                sx += x; sy += y; sz += zz; s2 += x*x + y*y + zz*zz;
+            }
+            const int64_t ex = r[3*(N-1)], ey = r[3*(N-1)+1], ez = r[3*(N-1)+2];
+            ree2 = (double)(ex*ex + ey*ey + ez*ez);
+            rg2  = (double)((int64_t)N * s2 - (sx*sx + sy*sy + sz*sz)) / ((double)N * (double)N);
+        } else {
+            lnW = -std::numeric_limits<double>::infinity();
+        }
+        res.push_back(ChainResult{lnW, ree2, rg2, alive});
+        dxor ^= h; dsum += h;
+        if (out) {
+            if (out->lnW) out->lnW[i] = lnW;
+            if (out->alive) out->alive[i] = alive ? 1 : 0;
+            if (out->digest) out->digest[i] = h;
+            if (out->ree2) out->ree2[i] = ree2;
+            if (out->rg2) out->rg2[i] = rg2;
+            if (out->conf) std::memcpy((int32_t*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(int32_t));
+        }
+    }
+    ensemble(summary, res, true, 0.0, n_steps, dxor, dsum);             // shift = largest lnW of the call (reading A18)
+    return 0;
+}
+
+// Real space with a square-well attraction: trial t overlaps as in Alg. 2 (d2 < sigma2); a free trial
+// carries Q[min(n_t, 31)], n_t = number of earlier monomers j <= s-2 with d2 < well2, well = fl32(lambda sigma),
+// well2 = fl32(well well), d2 the same fp32 expression as the overlap test. lambda >= 1.
+int oracle_realspace_model_generate(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                                    float lambda, double beta_eps, uint64_t seed, uint64_t chain_offset,
+                                    const oracle_outputs* out, oracle_summary* summary)
+{
+    if (N < 2 || n_chains == 0 || k_trials < 1 || k_trials > 255) return -1;
+    if (!(bond_len > 0.0f) || !(sigma >= 0.0f) || !std::isfinite(bond_len) || !std::isfinite(sigma)) return -1;
+    if (!(lambda >= 1.0f) || !std::isfinite(lambda) || !(beta_eps >= 0.0) || !(beta_eps <= 0.85)) return -1;
+    uint64_t Q[32];
+    oracle_model_table(beta_eps, Q);
+    const int32_t k = k_trials;
+    const float b = bond_len;
+    const float sigma2 = sigma * sigma;
+    const float well = lambda * sigma;
+    const float well2 = well * well;
+    std::vector<float> r((size_t)N * 3);
+    std::vector<float> trial((size_t)k * 3);
+    std::vector<uint64_t> w((size_t)k);
+    std::vector<ChainResult> res;
+    res.reserve(n_chains);
+    uint64_t n_steps = 0, dxor = 0, dsum = 0;
+
+    for (uint64_t i = 0; i < n_chains; ++i) {
+        const uint64_t chain = chain_offset + i;
+        std::fill(r.begin(), r.end(), 0.0f);
+        double lnW = 0.0;
+        bool alive = true;
+        uint64_t h = digest_init();
+        uint8_t* mrow = (out && out->m_seq) ? out->m_seq + i * (size_t)(N - 1) : nullptr;
+        if (mrow) std::memset(mrow, 0, (size_t)(N - 1));
+
+        for (int32_t s = 1; s <= N - 1; ++s) {
+            const float hx = r[3*(s-1)], hy = r[3*(s-1)+1], hz = r[3*(s-1)+2];
+            int32_t m = 0;
+            uint64_t W = 0;
+            for (int32_t t = 0; t < k; ++t) {
+                uint32_t wz, wphi; float u[3];
+                trial_words(seed, chain, (uint32_t)s, (uint32_t)t, &wz, &wphi);
+                oracle_direction(wz, wphi, u);
+                const float tx = std::fmaf(b, u[0], hx), ty = std::fmaf(b, u[1], hy), tz = std::fmaf(b, u[2], hz);
+                trial[3*t] = tx; trial[3*t+1] = ty; trial[3*t+2] = tz;
+                bool overlap = false;
+                int32_t n_well = 0;
+                for (int32_t j = 0; j < s - 1; ++j) {
+                    const float dx = r[3*j] - tx, dy = r[3*j+1] - ty, dz = r[3*j+2] - tz;
+                    const float d2 = std::fmaf(dz, dz, std::fmaf(dy, dy, dx * dx));
+                    if (d2 < sigma2) overlap = true;
+                    if (d2 < well2) ++n_well;
+                }
+                w[t] = overlap ? 0 : Q[n_well < 31 ? n_well : 31];
+                if (!overlap) ++m;
+                W += w[t];
+            }
+            ++n_steps;
+            if (mrow) mrow[s - 1] = (uint8_t)m;
+            if (m == 0) {
+                alive = false; h = digest_fold(h, 0, 0xFF);
+                for (int32_t q = s; q < N; ++q) r[3*q] = r[3*q+1] = r[3*q+2] = 0.0f;
+                break;
+            }
+            lnW += std::log((double)W * 0x1p-16);
+            const uint64_t target = scaled_target(selection_word(seed, chain, (uint32_t)s), W);
+            int32_t t = 0;
+            uint64_t cum = w[0];
+            while (cum <= target) cum += w[++t];
+            r[3*s] = trial[3*t]; r[3*s+1] = trial[3*t+1]; r[3*s+2] = trial[3*t+2];
+            h = digest_fold(h, (uint32_t)m, (uint32_t)t);
+        }
+
+        double ree2 = 0.0, rg2 = 0.0;
+        if (alive) {
+            double cx = 0.0, cy = 0.0, cz = 0.0;
+            for (int32_t q = 0; q < N; ++q) { cx += (double)r[3*q]; cy += (double)r[3*q+1]; cz += (double)r[3*q+2]; }
+            cx /= (double)N; cy /= (double)N; cz /= (double)N;
+            double acc = 0.0;
+            for (int32_t q = 0; q < N; ++q) {
+                const double ax = (double)r[3*q] - cx, ay = (double)r[3*q+1] - cy, az = (double)r[3*q+2] - cz;
+                acc += ax*ax + ay*ay + az*az;
+            }
+            rg2 = acc / (double)N;
+            const double ex = (double)r[3*(N-1)], ey = (double)r[3*(N-1)+1], ez = (double)r[3*(N-1)+2];
+            ree2 = ex*ex + ey*ey + ez*ez;
+        } else {
+            lnW = -std::numeric_limits<double>::infinity();
+        }
+        res.push_back(ChainResult{lnW, ree2, rg2, alive});
+        dxor ^= h; dsum += h;
+        if (out) {
+            if (out->lnW) out->lnW[i] = lnW;
+            if (out->alive) out->alive[i] = alive ? 1 : 0;
+            if (out->digest) out->digest[i] = h;
+            if (out->ree2) out->ree2[i] = ree2;
+            if (out->rg2) out->rg2[i] = rg2;
+            if (out->conf) std::memcpy((float*)out->conf + i * (size_t)N * 3, r.data(), (size_t)N * 3 * sizeof(float));
+        }
+    }
+    ensemble(summary, res, true, 0.0, n_steps, dxor, dsum);
+    return 0;
+}
+
 }  // extern "C"

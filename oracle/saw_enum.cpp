@@ -12,11 +12,15 @@
 //
 // The enumerator decides self-avoidance with its own grid, never with the oracle's scan.
 
+#include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
 extern "C" int32_t oracle_lattice_free_dirs(const int32_t* r, int32_t s, int32_t free_dirs[6]);
+extern "C" int32_t oracle_lattice_model_step(const int32_t* r, int32_t s, int32_t z, const uint64_t Q[32], uint64_t w[26]);
+extern "C" void oracle_model_table(double beta_eps, uint64_t Q[32]);
 
 namespace {
 
@@ -97,3 +101,82 @@ int oracle_saw_enumerate(int32_t n, int32_t fix_first, uint64_t* count, uint64_t
 }
 
 }  // extern "C"
+
+// Model enumerator (z = 6 or 26 trial set, contact energy): depth-first over all n-step SAWs with its OWN
+// occupancy grid, own direction table and own contact count (pairs |i - j| > 1 on neighbouring sites, counted from the
+// definition over the whole walk). For every walk w it accumulates
+//   count              1
+//   sum_boltz          q^contacts(w)                      (q = exp(beta_eps) in fp64: the exact partition sum Z_n)
+//   sum_boltz_ree2     q^contacts(w) Ree2(w)
+//   sum_quant          prod_s Q[c_s(w)] 2^-16              (what E[W] of the fixed-point Rosenbluth scheme converges to)
+//   sum_prob           prod_s w_s[d_s] / W_s               (probability that the ORACLE's step routine grows w;
+//                                                           summed over all walks = P_alive(n): non-statistical pin)
+// with c_s = contacts the monomer placed at step s makes; the last two use oracle_lattice_model_step (routine under test).
+namespace {
+struct EnumM {
+    int n, z, side;
+    std::vector<uint8_t> occ;
+    std::vector<int32_t> r;
+    uint64_t Q[32];
+    double q;
+    double count = 0, sum_boltz = 0, sum_boltz_ree2 = 0, sum_quant = 0, sum_prob = 0;
+    bool inconsistent = false;
+    int dirs[26][3];
+    size_t cell(int x, int y, int zc) const { return ((size_t)(x + n) * side + (size_t)(y + n)) * side + (size_t)(zc + n); }
+    bool adjacent(int i, int j) const {
+        const int dx = std::abs(r[3*i] - r[3*j]), dy = std::abs(r[3*i+1] - r[3*j+1]), dz = std::abs(r[3*i+2] - r[3*j+2]);
+        return z == 6 ? dx + dy + dz == 1 : (dx <= 1 && dy <= 1 && dz <= 1);
+    }
+    void grow(int s, double quant, double prob) {
+        if (s == n + 1) {
+            int contacts = 0;
+            for (int i = 0; i <= n; ++i) for (int j = i + 2; j <= n; ++j) if (adjacent(i, j)) ++contacts;
+            const double bw = std::pow(q, contacts);
+            const double x = r[3*n], y = r[3*n+1], zz = r[3*n+2];
+            count += 1; sum_boltz += bw; sum_boltz_ree2 += bw * (x*x + y*y + zz*zz); sum_quant += quant; sum_prob += prob;
+            return;
+        }
+        uint64_t w[26];
+        const int m = oracle_lattice_model_step(r.data(), s, z, Q, w);
+        uint64_t W = 0;
+        for (int d = 0; d < z; ++d) W += w[d];
+        int extended = 0;
+        for (int d = 0; d < z; ++d) {
+            const int x = r[3*(s-1)] + dirs[d][0], y = r[3*(s-1)+1] + dirs[d][1], zc = r[3*(s-1)+2] + dirs[d][2];
+            const size_t c = cell(x, y, zc);
+            if (occ[c]) { if (w[d] != 0) inconsistent = true; continue; }
+            if (w[d] == 0) { inconsistent = true; continue; }
+            ++extended;
+            occ[c] = 1; r[3*s] = x; r[3*s+1] = y; r[3*s+2] = zc;
+            grow(s + 1, quant * ((double)w[d] * 0x1p-16), prob * ((double)w[d] / (double)W));
+            occ[c] = 0;
+        }
+        if (extended != m) inconsistent = true;
+    }
+};
+}  // namespace
+
+extern "C" int oracle_saw_enumerate_model(int32_t n, int32_t z, double beta_eps, double out[5])
+{
+    if (n < 1 || n > 12 || (z != 6 && z != 26) || !out) return -1;
+    EnumM e;
+    e.n = n; e.z = z; e.side = 2 * n + 1; e.q = std::exp(beta_eps);
+    oracle_model_table(beta_eps, e.Q);
+    // own direction table, written out independently of the oracle's model_dir
+    int nd = 0;
+    if (z == 6) {
+        const int E6[6][3] = { {1,0,0}, {-1,0,0}, {0,1,0}, {0,-1,0}, {0,0,1}, {0,0,-1} };
+        for (; nd < 6; ++nd) for (int a = 0; a < 3; ++a) e.dirs[nd][a] = E6[nd][a];
+    } else {
+        for (int dz = -1; dz <= 1; ++dz) for (int dy = -1; dy <= 1; ++dy) for (int dx = -1; dx <= 1; ++dx) {
+            if (dx == 0 && dy == 0 && dz == 0) continue;
+            e.dirs[nd][0] = dx; e.dirs[nd][1] = dy; e.dirs[nd][2] = dz; ++nd;
+        }
+    }
+    e.occ.assign((size_t)e.side * e.side * e.side, 0);
+    e.r.assign((size_t)(n + 1) * 3, 0);
+    e.occ[e.cell(0, 0, 0)] = 1;
+    e.grow(1, 1.0, 1.0);
+    out[0] = e.count; out[1] = e.sum_boltz; out[2] = e.sum_boltz_ree2; out[3] = e.sum_quant; out[4] = e.sum_prob;
+    return e.inconsistent ? -2 : 0;
+}
