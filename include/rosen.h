@@ -126,6 +126,32 @@ ROSEN_API int rosen_realspace_generate(int32_t N, uint64_t n_chains, int32_t k_t
                              const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
 
 /*
+ * Other trial sets and Boltzmann-weighted trials (readings A19-A21).
+ *
+ * Lattice: z = 6 (the order above) or z = 26, "all z = 26 possible lattice space" (sec. 3.3.2): the 26 sites
+ * (dx,dy,dz) in {-1,0,1}^3 \ {0} around r_{s-1}, trial d = rank of (dx+1) + 3(dy+1) + 9(dz+1), site exclusion only.
+ * Energy U = -eps per non-bonded contact (Eq. 1-2): a free trial t whose site has c_t earlier monomers
+ * j <= s-2 on its z neighbour sites carries Q[c_t], Q[c] = round(q^c 2^16), q = exp(beta_eps) (fixed point: exact sums);
+ * W_s = sum_t Q[c_t]; the trial taken is the first, in trial order, whose cumulative sum exceeds floor(u_s W_s / 2^32);
+ * lnW += log(W_s 2^-16). m_seq = number of free trials; the chain is dead when that is 0. beta_eps = 0 reproduces
+ * rosen_lattice_generate decision for decision. 2 <= N <= ROSEN_LATTICE_MODEL_MAX_N, 0 <= beta_eps <= ROSEN_MODEL_MAX_BETA_EPS.
+ * summary->ln_shift is the largest lnW of the call. Uses 40 bytes per chain of library workspace (rosen_workspace_release).
+ *
+ * Real space: square well of range lambda sigma (lambda >= 1) and depth eps around every monomer: c_t = number of earlier
+ * monomers j <= s-2 with d2 < fl32(fl32(lambda sigma)^2), d2 the fp32 expression of the overlap test, capped at 31; the
+ * rest as on the lattice. 2 <= N <= ROSEN_REALSPACE_MODEL_MAX_N.
+ */
+#define ROSEN_LATTICE_MODEL_MAX_N    256
+#define ROSEN_REALSPACE_MODEL_MAX_N  399
+#define ROSEN_MODEL_MAX_BETA_EPS     0.85
+ROSEN_API int rosen_lattice_generate_model(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                                 int32_t z, double beta_eps,
+                                 const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
+ROSEN_API int rosen_realspace_generate_model(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma,
+                                   float lambda, double beta_eps, uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
+
+/*
  * Enqueue-only variants: same computation, but nothing is synchronised. All outputs must be device
  * memory (outputs->memory == ROSEN_MEM_DEVICE, else ROSEN_EINVAL); `summary_device` is a DEVICE
  * pointer (may be NULL) that the second reduction pass fills on `cuda_stream`, derived fields

@@ -83,6 +83,12 @@ def load_library() -> C.CDLL:
     L.rosen_fit_exponents.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_double), i32, i32,
                                       C.POINTER(rosen_fit)]
     L.rosen_fit_exponents.restype = C.c_int
+    L.rosen_lattice_generate_model.argtypes = [i32, u64, u64, u64, i32, C.c_double, C.POINTER(rosen_outputs),
+                                               C.POINTER(rosen_summary), vp]
+    L.rosen_lattice_generate_model.restype = C.c_int
+    L.rosen_realspace_generate_model.argtypes = [i32, u64, i32, C.c_float, C.c_float, C.c_float, C.c_double, u64, u64,
+                                                 C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
+    L.rosen_realspace_generate_model.restype = C.c_int
     L.rosen_direction_eval.argtypes = [vp, vp, u64, vp, i32, vp]
     L.rosen_direction_eval.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
@@ -181,6 +187,34 @@ def rosen_realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: flo
     _check(L.rosen_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, C.byref(st),
                                       C.byref(s) if summary else None, _stream_ptr(stream)))
     return (s.as_dict() if summary else None), tensors
+
+
+def rosen_lattice_generate_model(N: int, n_chains: int, seed: int, z: int = 6, beta_eps: float = 0.0, chain_offset: int = 0,
+                                 outputs: Iterable[str] = (), stream=None, host_outputs: bool = False):
+    """rosen_lattice_generate_model of include/rosen.h (z = 6 / 26 trial set, contact energy). Returns (summary, tensors)."""
+    L = load_library()
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
+    tensors, st = _alloc_outputs(N, n_chains, "int32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
+    s = rosen_summary()
+    _check(L.rosen_lattice_generate_model(N, n_chains, seed, chain_offset, z, beta_eps, C.byref(st), C.byref(s), _stream_ptr(stream)))
+    return s.as_dict(), tensors
+
+
+def rosen_realspace_generate_model(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, lam: float,
+                                   beta_eps: float, seed: int, chain_offset: int = 0, outputs: Iterable[str] = (),
+                                   stream=None, host_outputs: bool = False):
+    """rosen_realspace_generate_model of include/rosen.h (square well of range lam * sigma). Returns (summary, tensors)."""
+    L = load_library()
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
+    tensors, st = _alloc_outputs(N, n_chains, "float32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
+    s = rosen_summary()
+    _check(L.rosen_realspace_generate_model(N, n_chains, k_trials, bond_len, sigma, lam, beta_eps, seed, chain_offset,
+                                            C.byref(st), C.byref(s), _stream_ptr(stream)))
+    return s.as_dict(), tensors
 
 
 SUMMARY_BYTES = C.sizeof(rosen_summary)

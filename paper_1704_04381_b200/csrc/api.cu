@@ -339,6 +339,96 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
     return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, outputs, z, st, summary, summary_dev, stream);
 }
 
+// Fixed-point Boltzmann factors of the model calls: Q[c] = round(p_c 2^16), p_0 = 1, p_c = p_{c-1} q in fp64.
+void model_table(double beta_eps, uint64_t Q[32])
+{
+    const double q = std::exp(beta_eps);
+    double pw = 1.0;
+    for (int c = 0; c < 32; ++c) { Q[c] = (uint64_t)std::llround(pw * 65536.0); pw *= q; }
+}
+
+int lattice_model_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, int32_t z, double beta_eps,
+                       const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_chains == 0 || (z != 6 && z != 26) || !(beta_eps >= 0.0) || !(beta_eps <= ROSEN_MODEL_MAX_BETA_EPS)) {
+        std::snprintf(g_err, sizeof(g_err), "need N >= 2, n_chains >= 1, z = 6 or 26, 0 <= beta_eps <= %.2f", ROSEN_MODEL_MAX_BETA_EPS);
+        return ROSEN_EINVAL;
+    }
+    if (N > ROSEN_LATTICE_MODEL_MAX_N) { std::snprintf(g_err, sizeof(g_err), "lattice model N > %d", ROSEN_LATTICE_MODEL_MAX_N); return ROSEN_ERANGE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* sc = nullptr;
+    int rc = get_scratch(&sc);
+    if (rc) return rc;
+    const Sizes zs = output_sizes(N, n_chains, sizeof(int32_t));
+    Staging st;
+    if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;
+    rosen::ModelParams mp{};
+    mp.N = N; mp.z = z; mp.n_chains = n_chains; mp.chain_offset = chain_offset;
+    mp.key0 = (uint32_t)seed; mp.key1 = (uint32_t)(seed >> 32);
+    model_table(beta_eps, mp.Q);
+    mp.out = st.dev; mp.partials = sc->dev;
+    rosen::partition_chains(n_chains, &mp.chunk, &mp.n_vblocks, 256u);
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
+    }
+    mp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
+    mp.lmax = sc->lmax;
+    rc = rosen::launch_lattice_model(mp, stream, &g_kernel);
+    if (rc < 0) return fail_cuda(cudaGetLastError(), "lattice model kernel launch");
+    g_launches += rc;
+    return finish(sc, (int)mp.n_vblocks, n_chains, 0.0, mp.lmax + rosen::kMaxPartials, outputs, zs, st, summary, nullptr, stream);
+}
+
+int realspace_model_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma, float lambda, double beta_eps,
+                         uint64_t seed, uint64_t chain_offset, const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_chains == 0 || k_trials < 1 || k_trials > 255 || !(bond_len > 0.0f) || !(sigma >= 0.0f) ||
+        !std::isfinite(bond_len) || !std::isfinite(sigma) || !(lambda >= 1.0f) || !std::isfinite(lambda) ||
+        !(beta_eps >= 0.0) || !(beta_eps <= ROSEN_MODEL_MAX_BETA_EPS)) {
+        std::snprintf(g_err, sizeof(g_err), "need N >= 2, n_chains >= 1, 1 <= k_trials <= 255, bond_len > 0, sigma >= 0, lambda >= 1 (finite), 0 <= beta_eps <= %.2f",
+                      ROSEN_MODEL_MAX_BETA_EPS);
+        return ROSEN_EINVAL;
+    }
+    if (N > ROSEN_REALSPACE_MODEL_MAX_N) { std::snprintf(g_err, sizeof(g_err), "real-space model N > %d", ROSEN_REALSPACE_MODEL_MAX_N); return ROSEN_ERANGE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* sc = nullptr;
+    int rc = get_scratch(&sc);
+    if (rc) return rc;
+    const Sizes zs = output_sizes(N, n_chains, sizeof(float));
+    Staging st;
+    if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;
+    const float well = lambda * sigma;              // fp32 products, rounded once each
+    rosen::RealParams p{};
+    p.N = N; p.k = k_trials; p.n_chains = n_chains; p.chain_offset = chain_offset;
+    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
+    p.b = bond_len; p.sigma2 = sigma * sigma; p.well2 = well * well;
+    // conservative candidate radius around the well instead of the core: ((b + lambda sigma)(1 + 2^-9))^2, rounded up
+    const double cand_r = ((double)bond_len + (double)well) * (1.0 + 1.0 / 512.0);
+    p.prefilter2 = (float)(cand_r * cand_r);
+    if ((double)p.prefilter2 < cand_r * cand_r) p.prefilter2 = std::nextafterf(p.prefilter2, INFINITY);
+    p.ln_shift = 0.0;
+    model_table(beta_eps, p.Q);
+    p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
+    rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks, 256u);
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
+    }
+    p.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
+    CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));
+    int grid = 0;
+    rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
+    if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space model kernel launch");
+    g_launches += rc;
+    rc = rosen::launch_reduce_records(p.rec, n_chains, p.chunk, p.n_vblocks, 0.0, sc->lmax, st.dev, sc->dev, stream);
+    if (rc < 0) return fail_cuda(cudaGetLastError(), "record reduction");
+    g_launches += rc;
+    return finish(sc, (int)p.n_vblocks, n_chains, 0.0, sc->lmax + rosen::kMaxPartials, outputs, zs, st, summary, nullptr, stream);
+}
+
 }  // namespace
 
 extern "C" {
@@ -390,6 +480,19 @@ int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trials, float b
     rosen_outputs o{};
     o.conf = conf; o.lnW = lnW; o.memory = memory;
     return rosen_realspace_generate(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, &o, summary, cuda_stream);
+}
+
+int rosen_lattice_generate_model(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, int32_t z, double beta_eps,
+                                 const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    return lattice_model_impl(N, n_chains, seed, chain_offset, z, beta_eps, outputs, summary, cuda_stream);
+}
+
+int rosen_realspace_generate_model(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_len, float sigma, float lambda,
+                                   double beta_eps, uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    return realspace_model_impl(N, n_chains, k_trials, bond_len, sigma, lambda, beta_eps, seed, chain_offset, outputs, summary, cuda_stream);
 }
 
 int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged)

@@ -36,6 +36,7 @@ struct LatticeParams {
                                 // partials[v] never depends on which block computed it)
 };
 
+struct ChainRecord;
 struct RealParams {
     int32_t    N;
     int32_t    k;
@@ -49,6 +50,10 @@ struct RealParams {
     uint32_t   chunk;           // chains per virtual block (multiple of 256)
     uint32_t   n_vblocks;
     uint32_t*  vb_counter;      // as in LatticeParams
+    // square-well model (rosen_realspace_generate_model): rec != nullptr selects the WELL kernels
+    float        well2;         // fl32(fl32(lambda sigma)^2)
+    ChainRecord* rec;           // [n_chains]: per-chain records instead of block partials (shift = largest lnW of the call)
+    uint64_t     Q[32];         // fixed-point Boltzmann factors round(q^c 2^16)
 };
 
 // Long-chain lattice path (lattice_hash.cu): one fixed-size record per chain, reduced afterwards in a fixed order.
@@ -73,6 +78,22 @@ struct HashParams {
     uint32_t   entries;         // entries per chain table (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
     double*    lmax;            // [kMaxPartials + 1] scratch, or null: N <= 512, fixed shift ln_shift (reading A18)
+};
+
+// Lattice model path (lattice_model.cu): z = 6 / 26 trial set, contact energy, records + dynamic shift.
+struct ModelParams {
+    int32_t    N;
+    int32_t    z;
+    uint64_t   n_chains;
+    uint64_t   chain_offset;
+    uint32_t   key0, key1;
+    uint64_t   Q[32];           // fixed-point Boltzmann factors round(q^c 2^16)
+    DevOutputs out;
+    Partial*   partials;        // [n_vblocks]
+    uint32_t   chunk;
+    uint32_t   n_vblocks;
+    ChainRecord* rec;           // [n_chains]
+    double*    lmax;            // [kMaxPartials + 1] scratch of the max pass
 };
 
 constexpr uint32_t kRealLongCandCap = 160;
@@ -134,6 +155,8 @@ int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t ch
 int real_long_max_warps(int k, int* warps_out);
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
+// lattice_model.cu: generation kernel + record reduction (max pass included); returns the launches made
+int launch_lattice_model(const ModelParams& p, cudaStream_t stream, const char** kernel_name);
 // realspace.cu: the direction map of DESIGN.md 3.3 alone, out[3 i ..] = direction(wz[i], wphi[i]) (device pointers)
 int launch_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* out, cudaStream_t stream);
 int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift, const double* ln_shift_dev,

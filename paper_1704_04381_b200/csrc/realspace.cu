@@ -22,6 +22,7 @@ namespace rosen {
 
 namespace {
 
+constexpr size_t kFixedBytes = 256 * sizeof(double) + 32 * sizeof(Partial) + 32 * sizeof(uint64_t);   // ln_tab | scratch | Q
 constexpr float kFar = 1.0e18f;   // sentinel coordinate: squared distances ~3e36 stay finite and fail every test
 
 // shared memory carve-up (bytes) -----------------------------------------------------------------
@@ -106,7 +107,10 @@ __device__ __forceinline__ uint32_t candidate_bits(const float4* base, int cnt, 
 
 // MSEQ: the per-step m sequence is requested (one shared-memory byte per step). The conformation dump needs no
 // variant: the chain is in shared memory anyway and is stored once, after the last step, if p.out.conf is set.
-template <int G, int P, bool DIGEST, bool MSEQ>
+// WELL: square-well model of DESIGN.md 3.6 (rosen_realspace_generate_model): contacts inside lambda sigma are counted
+// per trial, the trial factors are the fixed-point Q[c], the choice is proportional to them, and the chain's result goes to
+// a record (reduced afterwards with the largest lnW of the call as the shift) instead of the block partial.
+template <int G, int P, bool DIGEST, bool MSEQ, bool WELL>
 __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
 {
     constexpr int T = 2 * P;                                 // trials per lane: t = T * gl + i, i = 0..T-1
@@ -114,7 +118,8 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* ln_tab = reinterpret_cast<double*>(smem_raw);
     Partial* scratch = reinterpret_cast<Partial*>(smem_raw + 256 * sizeof(double));
-    unsigned char* gbase_ptr = smem_raw + 256 * sizeof(double) + 32 * sizeof(Partial);
+    uint64_t* Qs = reinterpret_cast<uint64_t*>(smem_raw + 256 * sizeof(double) + 32 * sizeof(Partial));
+    unsigned char* gbase_ptr = smem_raw + kFixedBytes;
 
     const int N = p.N, k = p.k, Np = n_pad(N);
     const int lane = threadIdx.x & 31;
@@ -127,6 +132,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
     uint8_t* mbuf = reinterpret_cast<uint8_t*>(R4 + Np);
 
     for (int i = threadIdx.x; i < 256; i += blockDim.x) ln_tab[i] = i == 0 ? -CUDART_INF : log((double)i);
+    if (threadIdx.x < 32) Qs[threadIdx.x] = p.Q[threadIdx.x];
     __syncthreads();
 
     // Virtual blocks (common.cuh): virtual block vb owns chains [vb*chunk, (vb+1)*chunk); group g of the block takes
@@ -173,6 +179,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             // ---- R1: this lane's trials (P Philox blocks = 2P consecutive trials)
             float tx[T], ty[T], tz[T];
             float near2[T];                                  // smallest spec'd d2 to an earlier monomer so far (-1: trial index >= k)
+            uint32_t nwell[T];                               // WELL: earlier monomers with d2 < well2
 #pragma unroll
             for (int pp = 0; pp < P; ++pp) {
                 const uint32_t bi = (uint32_t)(P * gl + pp);
@@ -186,6 +193,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
                     ty[2 * pp + e] = __fmaf_rn(p.b, uy, hy);
                     tz[2 * pp + e] = __fmaf_rn(p.b, uz, hz);
                     near2[2 * pp + e] = (int)(2u * bi + e) < k ? CUDART_MAX_NORMAL_F : -1.0f;
+                    nwell[2 * pp + e] = 0u;
                 }
             }
 
@@ -204,6 +212,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
                         const float dx = __fsub_rn(rj.x, tx[i]), dy = __fsub_rn(rj.y, ty[i]), dz = __fsub_rn(rj.z, tz[i]);
                         const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                         near2[i] = fminf(near2[i], d2);      // overlap iff some d2 < sigma2 iff the smallest is
+                        if (WELL) nwell[i] += d2 < p.well2 ? 1u : 0u;
                     }
                 }
             }
@@ -234,17 +243,45 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
 
             // ---- R3
             steps += alive ? 1u : 0u;
-            lnW += ln_tab[m];
             if (MSEQ) { if (gl == 0) mbuf[s - 1] = alive ? (uint8_t)m : (uint8_t)0; }
 
-            // ---- R4: the sel-th free trial; it is this lane's if excl <= sel < excl + c, namely the (sel - excl)-th set bit of f
-            const uint32_t sel = __umulhi(usel, m);
-            const uint32_t rk = sel - excl;
-            const bool hit = rk < c;
-            uint32_t g2 = f;
+            // ---- R4
+            bool hit;
+            int li;
+            if constexpr (!WELL) {
+                lnW += ln_tab[m];
+                // the sel-th free trial; it is this lane's if excl <= sel < excl + c, namely the (sel - excl)-th set bit of f
+                const uint32_t sel = __umulhi(usel, m);
+                const uint32_t rk = sel - excl;
+                hit = rk < c;
+                uint32_t g2 = f;
 #pragma unroll
-            for (int i = 0; i < T - 1; ++i) g2 = (rk > (uint32_t)i) ? (g2 & (g2 - 1u)) : g2;
-            const int li = __ffs(g2) - 1;
+                for (int i = 0; i < T - 1; ++i) g2 = (rk > (uint32_t)i) ? (g2 & (g2 - 1u)) : g2;
+                li = __ffs(g2) - 1;
+            } else {
+                // Boltzmann-weighted choice: integer factors, so the group's prefix sums are exact
+                uint64_t lw[T], Ls = 0;
+#pragma unroll
+                for (int i = 0; i < T; ++i) { lw[i] = ((f >> i) & 1u) ? Qs[min(nwell[i], 31u)] : 0ull; Ls += lw[i]; }
+                uint64_t inc = Ls;
+#pragma unroll
+                for (int d = 1; d < G; d <<= 1) {
+                    const uint64_t v = __shfl_up_sync(kFull, (unsigned long long)inc, d, G);
+                    if (gl >= d) inc += v;
+                }
+                const uint64_t Wt = G > 1 ? (uint64_t)__shfl_sync(kFull, (unsigned long long)inc, gshift + G - 1) : inc;
+                lnW += log((double)Wt * 0x1p-16);            // log(0) = -inf for a dead end
+                const uint64_t target = (Wt >> 32) * (uint64_t)usel + (((Wt & 0xFFFFFFFFull) * (uint64_t)usel) >> 32);
+                uint64_t cum = inc - Ls;
+                hit = Wt != 0ull && target >= cum && target < inc;
+                li = T - 1;
+                bool found = false;
+#pragma unroll
+                for (int i = 0; i < T; ++i) {
+                    cum += lw[i];
+                    if (!found && cum > target) { found = true; li = i; }
+                }
+            }
             float px = tx[0], py = ty[0], pz = tz[0];
 #pragma unroll
             for (int i = 1; i < T; ++i)
@@ -285,8 +322,15 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             const double cx = Sx * inv, cy = Sy * inv, cz = Sz * inv;
             rg2 = S2 * inv - (cx * cx + cy * cy + cz * cz);
         }
-        const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
-        if (active && gl == 0) {
+        const double wgt = (alive && !WELL) ? exp(lnW - p.ln_shift) : 0.0;
+        if (WELL) {
+            if (active && gl == 0) {
+                ChainRecord rc;
+                rc.lnW = alive ? lnW : -CUDART_INF; rc.ree2 = ree2; rc.rg2 = rg2;
+                rc.steps = steps; rc.alive = alive ? 1u : 0u; rc.digest = dg;
+                p.rec[idx] = rc;
+            }
+        } else if (active && gl == 0) {
             acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
             acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
             if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
@@ -328,32 +372,33 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
         __syncwarp();
     }
 
-    block_reduce_store(acc, scratch, p.partials + vb);
+    if (WELL) __syncthreads();      // the sums are formed from the records afterwards; the ticket still needs the barrier
+    else block_reduce_store(acc, scratch, p.partials + vb);
     }
 }
 
 // threads per block: a function of (N, G) only -- it fixes the reduction tree, so it must not depend on the output variant
 int block_threads(int N, int G)
 {
-    const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
+    const size_t fixed = kFixedBytes;
     const size_t gsz = group_bytes(N, G, true);
     int threads = 256;
     while (threads > 32 && fixed + gsz * (threads / G) > (size_t)(74 * 1024 + 512)) threads >>= 1;   // three blocks per SM
     return threads;
 }
 
-template <int G, int P, bool DIGEST, bool MSEQ>
+template <int G, int P, bool DIGEST, bool MSEQ, bool WELL>
 int launch_one(const RealParams& p, cudaStream_t stream, int* grid_out)
 {
     int dev = 0, n_sm = 0, smem_max = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const size_t fixed = 256 * sizeof(double) + 32 * sizeof(Partial);
+    const size_t fixed = kFixedBytes;
     const int threads = block_threads(p.N, G);
     const size_t smem = fixed + group_bytes(p.N, G, MSEQ) * (threads / G);
     if (smem > (size_t)smem_max) return -2;
-    auto kern = realspace_kernel<G, P, DIGEST, MSEQ>;
+    auto kern = realspace_kernel<G, P, DIGEST, MSEQ, WELL>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
@@ -371,8 +416,10 @@ int launch_gp(const RealParams& p, cudaStream_t stream, int* grid_out)
 {
     const bool digest = p.out.digest != nullptr;
     const bool mseq = p.out.m_seq != nullptr;
-    if (mseq) return digest ? launch_one<G, P, true, true>(p, stream, grid_out) : launch_one<G, P, false, true>(p, stream, grid_out);
-    return digest ? launch_one<G, P, true, false>(p, stream, grid_out) : launch_one<G, P, false, false>(p, stream, grid_out);
+    if (p.rec != nullptr)          // square-well model: the record always carries the digest
+        return mseq ? launch_one<G, P, true, true, true>(p, stream, grid_out) : launch_one<G, P, true, false, true>(p, stream, grid_out);
+    if (mseq) return digest ? launch_one<G, P, true, true, false>(p, stream, grid_out) : launch_one<G, P, false, true, false>(p, stream, grid_out);
+    return digest ? launch_one<G, P, true, false, false>(p, stream, grid_out) : launch_one<G, P, false, false, false>(p, stream, grid_out);
 }
 
 // direction map alone (test entry rosen_direction_eval): out[3 i ..] = direction(wz[i], wphi[i])
