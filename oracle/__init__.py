@@ -70,6 +70,9 @@ def lib() -> C.CDLL:
         L.oracle_realspace_model_generate.restype = C.c_int
         L.oracle_saw_enumerate_model.argtypes = [C.c_int32, C.c_int32, C.c_double, C.POINTER(C.c_double)]
         L.oracle_saw_enumerate_model.restype = C.c_int
+        L.oracle_lattice_perm.argtypes = [C.c_int32, C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(C.c_double),
+                                          C.POINTER(C.c_double), C.c_double, C.c_uint64, C.POINTER(_Outputs), C.POINTER(_Summary)]
+        L.oracle_lattice_perm.restype = C.c_int
         _LIB = L
     return _LIB
 
@@ -173,6 +176,21 @@ def saw_enumerate_model(n: int, z: int, beta_eps: float) -> dict:
     if rc != 0:
         raise RuntimeError(f"oracle_saw_enumerate_model rc={rc}")
     return dict(zip(("count", "sum_boltz", "sum_boltz_ree2", "sum_quant", "sum_prob"), [float(v) for v in out]))
+
+
+def lattice_perm(N: int, n_tours: int, seed: int, ln_lo, ln_hi, ln_ref: float, max_nodes: int = 1 << 20, tour_offset: int = 0,
+                 outputs=("lnW", "alive", "digest", "ree2", "rg2")) -> Result:
+    """PERM tours on the cubic lattice with caller-given thresholds ln_lo / ln_hi [N+1] (index = number of monomers,
+    entries 2..N-1 used); per-tour results in the per-chain fields (see rosen_oracle.cpp)."""
+    lo = np.ascontiguousarray(ln_lo, dtype=np.float64); hi = np.ascontiguousarray(ln_hi, dtype=np.float64)
+    assert lo.shape == (N + 1,) and hi.shape == (N + 1,)
+    arrs, out = _alloc(n_tours, N, np.int32, set(outputs) - {"conf", "m_seq"})
+    s = _Summary()
+    rc = lib().oracle_lattice_perm(N, n_tours, seed, tour_offset, lo.ctypes.data_as(C.POINTER(C.c_double)),
+                                   hi.ctypes.data_as(C.POINTER(C.c_double)), ln_ref, max_nodes, C.byref(out), C.byref(s))
+    if rc != 0:
+        raise ValueError(f"oracle_lattice_perm: invalid arguments (rc={rc})")
+    return Result(summary=_summary_dict(s), **arrs)
 
 
 def philox4x32_10(ctr, key) -> tuple:

@@ -620,4 +620,105 @@ int oracle_realspace_model_generate(int32_t N, uint64_t n_chains, int32_t k_tria
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// PERM, the pruned-enriched Rosenbluth method. The paper names it only as the topic of its
+// supplement ("Parallel implementation of PERM on GPU"), which is not available: what follows is the
+// published algorithm (P. Grassberger, Phys. Rev. E 56, 3682 (1997)) in its depth-first recursive form, with the
+// population-control thresholds GIVEN by the caller (readings A22-A24) so that a tour is a pure function
+// of (seed, tour id, thresholds):
+//   step(n, lnW): the chain has n monomers and weight W. If n = N it is a leaf: the tour's sums take W, W Ree2, W Rg2.
+//     Otherwise node = next node number of the tour; m = free neighbours (Alg. 1); m = 0: dead end, return.
+//     W' = W m; the monomer goes to the ((u m) >> 32)-th free site, u = selection word (seed, tour, node + 1) of 3.1.
+//     Population control at the new length n + 1 < N:  lnW' > ln_hi[n+1]: enrichment, two copies of weight W'/2 each;
+//     lnW' < ln_lo[n+1]: pruning, killed if the coin word (Philox counter (tour, node >> 2, 2), word node & 3) is < 2^31,
+//     else the weight doubles. Then step(n + 1, .) once per copy. A tour that reaches max_nodes nodes stops (flag 2).
+// With ln_lo = -inf, ln_hi = +inf a tour IS the Rosenbluth chain of the same id (same words, same decisions).
+// The estimate of Z_N is the mean over tours of S = sum of leaf weights; E[S] = c_{N-1} for any thresholds.
+// ---------------------------------------------------------------------------------------------
+struct PermTour {
+    int32_t N; uint64_t seed, tour; const double* ln_lo; const double* ln_hi; double ln_ref; uint64_t max_nodes;
+    std::vector<int32_t> r;
+    uint64_t node = 0, leaves = 0, h = 0;
+    bool capped = false;
+    double S = 0.0, SR = 0.0, SG = 0.0;       // sums of exp(lnW - ln_ref) (x Ree2, x Rg2) over the leaves, depth-first order
+
+    void step(int32_t n, double lnW) {
+        if (capped) return;
+        if (n == N) {
+            int64_t sx = 0, sy = 0, sz = 0, s2 = 0;
+            for (int32_t q = 0; q < N; ++q) {
+                const int64_t x = r[3*q], y = r[3*q+1], z = r[3*q+2];
+                sx += x; sy += y; sz += z; s2 += x*x + y*y + z*z;
+            }
+            const int64_t ex = r[3*(N-1)], ey = r[3*(N-1)+1], ez = r[3*(N-1)+2];
+            const double ree2 = (double)(ex*ex + ey*ey + ez*ez);
+            const double rg2 = (double)((int64_t)N * s2 - (sx*sx + sy*sy + sz*sz)) / ((double)N * (double)N);
+            const double w = std::exp(lnW - ln_ref);
+            S += w; SR += w * ree2; SG += w * rg2; ++leaves;
+            return;
+        }
+        if (node >= max_nodes) { capped = true; return; }
+        const uint64_t id = node++;
+        int32_t free_dirs[6];
+        const int32_t m = oracle_lattice_free_dirs(r.data(), n, free_dirs);
+        if (m == 0) { h = digest_fold(h, 0, 0xFF); return; }
+        lnW += std::log((double)m);
+        const uint32_t u = selection_word(seed, tour, (uint32_t)(id + 1));
+        const int32_t d = free_dirs[(uint32_t)(((uint64_t)u * (uint64_t)m) >> 32)];
+        for (int a = 0; a < 3; ++a) r[3*n+a] = r[3*(n-1)+a] + E[d][a];
+        int copies = 1;
+        uint32_t event = 0;
+        if (n + 1 < N) {
+            if (lnW > ln_hi[n + 1]) { copies = 2; lnW -= std::log(2.0); event = 1; }
+            else if (lnW < ln_lo[n + 1]) {
+                const uint32_t ctr[4] = { (uint32_t)tour, (uint32_t)(tour >> 32), (uint32_t)(id >> 2), 2u };
+                const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+                uint32_t w4[4];
+                oracle_philox4x32_10(ctr, key, w4);
+                if (w4[id & 3u] < 0x80000000u) { copies = 0; event = 3; } else { lnW += std::log(2.0); event = 2; }
+            }
+        }
+        h = digest_fold(h, (uint32_t)m | (event << 4), (uint32_t)d);
+        for (int c = 0; c < copies; ++c) {
+            // the copy made at this length continues from r[0..n]; deeper levels only overwrote monomers > n
+            for (int a = 0; a < 3; ++a) r[3*n+a] = r[3*(n-1)+a] + E[d][a];
+            step(n + 1, lnW);
+        }
+    }
+};
+
+// Per-tour results use the per-chain fields: lnW = ln S (ln of the tour's summed leaf weights, -inf without a leaf),
+// ree2 / rg2 = the tour's weighted means SR/S, SG/S, alive = 1 (some leaf), 0 (none), 2 (stopped at max_nodes).
+// Summary: n_chains = tours, n_dead = tours without a leaf, n_steps_attempted = nodes, sums over tours of
+// exp(lnS - L) (x ree2, x rg2, squared), L = largest lnS; mean_* = W-weighted means over all leaves, ln_mean_W = ln Z_N estimate.
+int oracle_lattice_perm(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset, const double* ln_lo, const double* ln_hi,
+                        double ln_ref, uint64_t max_nodes, const oracle_outputs* out, oracle_summary* summary)
+{
+    if (N < 2 || N > 4096 || n_tours == 0 || !ln_lo || !ln_hi || max_nodes == 0 || !std::isfinite(ln_ref)) return -1;
+    std::vector<ChainResult> res;
+    res.reserve(n_tours);
+    uint64_t n_nodes = 0, dxor = 0, dsum = 0;
+    for (uint64_t i = 0; i < n_tours; ++i) {
+        PermTour t;
+        t.N = N; t.seed = seed; t.tour = tour_offset + i; t.ln_lo = ln_lo; t.ln_hi = ln_hi; t.ln_ref = ln_ref; t.max_nodes = max_nodes;
+        t.r.assign((size_t)N * 3, 0);
+        t.h = digest_init();
+        t.step(1, 0.0);
+        const bool have = t.S > 0.0;
+        const double lnS = have ? ln_ref + std::log(t.S) : -std::numeric_limits<double>::infinity();
+        const double ree2 = have ? t.SR / t.S : 0.0, rg2 = have ? t.SG / t.S : 0.0;
+        res.push_back(ChainResult{lnS, ree2, rg2, have});
+        n_nodes += t.node; dxor ^= t.h; dsum += t.h;
+        if (out) {
+            if (out->lnW) out->lnW[i] = lnS;
+            if (out->alive) out->alive[i] = t.capped ? 2 : (have ? 1 : 0);
+            if (out->digest) out->digest[i] = t.h;
+            if (out->ree2) out->ree2[i] = ree2;
+            if (out->rg2) out->rg2[i] = rg2;
+        }
+    }
+    ensemble(summary, res, true, 0.0, n_nodes, dxor, dsum);
+    return 0;
+}
+
 }  // extern "C"
