@@ -152,6 +152,27 @@ ROSEN_API int rosen_realspace_generate_model(int32_t N, uint64_t n_chains, int32
                                    const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
 
 /*
+ * PERM, the pruned-enriched Rosenbluth method, on the cubic lattice. The paper names
+ * it only as the topic of its supplement (not available); the algorithm is P. Grassberger's (Phys. Rev. E
+ * 56, 3682 (1997)), depth-first, one TOUR per id: the chain grows as in rosen_lattice_generate; after a step that brings it
+ * to n monomers (2 <= n <= N-1) with weight W, lnW > ln_hi[n] replaces it by two copies of weight W/2 (enrichment),
+ * lnW < ln_lo[n] kills it with probability 1/2 and doubles its weight otherwise (pruning); every chain of the tour that
+ * reaches N monomers is a leaf. ln_lo, ln_hi: HOST arrays of N+1 doubles (entries 2..N-1 are read; -inf / +inf switch
+ * the control off, and a tour is then exactly the chain of the same id). The estimate of Z_N is unbiased for any
+ * thresholds. ln_ref: leaf weights are summed inside a tour as exp(lnW - ln_ref) (choose ~ ln Z_N). A tour stops after
+ * max_nodes growth steps. Random words: DESIGN.md 3.7.
+ * Per-tour outputs (tour i has id tour_offset + i): lnW = ln(sum of its leaf weights), -inf without a leaf; ree2 / rg2 =
+ * its weight-averaged leaf observables; alive = 1 (some leaf), 0 (none), 2 (stopped at max_nodes); digest of its decisions;
+ * m_seq and conf must be NULL. Summary: n_chains = tours, n_dead = tours without a leaf, n_steps_attempted = growth steps
+ * of all tours, sums over tours of exp(lnW - ln_shift) with ln_shift = the largest lnW, mean_ree2 / mean_rg2 = weighted means
+ * over all leaves, ln_mean_W = estimate of ln Z_N (Eq. 6). 2 <= N <= ROSEN_PERM_MAX_N.
+ */
+#define ROSEN_PERM_MAX_N 512
+ROSEN_API int rosen_lattice_perm(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset,
+                       const double* ln_lo, const double* ln_hi, double ln_ref, uint32_t max_nodes,
+                       const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
+
+/*
  * Enqueue-only variants: same computation, but nothing is synchronised. All outputs must be device
  * memory (outputs->memory == ROSEN_MEM_DEVICE, else ROSEN_EINVAL); `summary_device` is a DEVICE
  * pointer (may be NULL) that the second reduction pass fills on `cuda_stream`, derived fields

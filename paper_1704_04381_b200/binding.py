@@ -89,6 +89,9 @@ def load_library() -> C.CDLL:
     L.rosen_realspace_generate_model.argtypes = [i32, u64, i32, C.c_float, C.c_float, C.c_float, C.c_double, u64, u64,
                                                  C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
     L.rosen_realspace_generate_model.restype = C.c_int
+    L.rosen_lattice_perm.argtypes = [i32, u64, u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, C.c_uint32,
+                                     C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
+    L.rosen_lattice_perm.restype = C.c_int
     L.rosen_direction_eval.argtypes = [vp, vp, u64, vp, i32, vp]
     L.rosen_direction_eval.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
@@ -214,6 +217,22 @@ def rosen_realspace_generate_model(N: int, n_chains: int, k_trials: int, bond_le
     s = rosen_summary()
     _check(L.rosen_realspace_generate_model(N, n_chains, k_trials, bond_len, sigma, lam, beta_eps, seed, chain_offset,
                                             C.byref(st), C.byref(s), _stream_ptr(stream)))
+    return s.as_dict(), tensors
+
+
+def rosen_lattice_perm(N: int, n_tours: int, seed: int, ln_lo, ln_hi, ln_ref: float, max_nodes: int = 1 << 20,
+                       tour_offset: int = 0, outputs: Iterable[str] = (), stream=None, host_outputs: bool = False):
+    """rosen_lattice_perm of include/rosen.h: ln_lo, ln_hi = sequences of N+1 floats. Returns (summary, tensors)."""
+    L = load_library()
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
+    if len(ln_lo) != N + 1 or len(ln_hi) != N + 1:
+        raise ValueError("ln_lo, ln_hi need N + 1 entries")
+    lo = (C.c_double * (N + 1))(*[float(v) for v in ln_lo]); hi = (C.c_double * (N + 1))(*[float(v) for v in ln_hi])
+    tensors, st = _alloc_outputs(N, n_tours, "int32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
+    s = rosen_summary()
+    _check(L.rosen_lattice_perm(N, n_tours, seed, tour_offset, lo, hi, ln_ref, max_nodes, C.byref(st), C.byref(s), _stream_ptr(stream)))
     return s.as_dict(), tensors
 
 

@@ -12,7 +12,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["api.cu", "lattice.cu", "lattice_hash.cu", "lattice_model.cu", "realspace.cu", "realspace_long.cu", "reduce.cu"]
+SOURCES = ["api.cu", "lattice.cu", "lattice_hash.cu", "lattice_model.cu", "lattice_perm.cu", "realspace.cu", "realspace_long.cu", "reduce.cu"]
 HEADERS = ["common.cuh", "direction.cuh", "philox.cuh", "reduce.cuh", os.path.join("..", "..", "include", "rosen.h")]
 TARGET = os.path.join(HERE, "librosen.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

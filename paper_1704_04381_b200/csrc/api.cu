@@ -38,6 +38,7 @@ struct Scratch {
     void*          hash_tables = nullptr;  size_t hash_tables_bytes = 0;
     void*          hash_rec = nullptr;     size_t hash_rec_bytes = 0;
     unsigned long long* hash_ticket = nullptr;
+    double*        perm_thr = nullptr;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
 };
 constexpr size_t kHashTableCap = (size_t)12 << 30;  // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
@@ -429,6 +430,48 @@ int realspace_model_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float b
     return finish(sc, (int)p.n_vblocks, n_chains, 0.0, sc->lmax + rosen::kMaxPartials, outputs, zs, st, summary, nullptr, stream);
 }
 
+int perm_impl(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset, const double* ln_lo, const double* ln_hi,
+              double ln_ref, uint32_t max_nodes, const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_tours == 0 || !ln_lo || !ln_hi || max_nodes == 0 || !std::isfinite(ln_ref) ||
+        (outputs && (outputs->m_seq || outputs->conf))) {
+        std::snprintf(g_err, sizeof(g_err), "need N >= 2, n_tours >= 1, thresholds, max_nodes >= 1, finite ln_ref; per-tour outputs are lnW, alive, digest, ree2, rg2");
+        return ROSEN_EINVAL;
+    }
+    for (int32_t n = 2; n < N && n <= ROSEN_PERM_MAX_N; ++n)
+        if (std::isnan(ln_lo[n]) || std::isnan(ln_hi[n])) { std::snprintf(g_err, sizeof(g_err), "NaN threshold at length %d", n); return ROSEN_EINVAL; }
+    if (N > ROSEN_PERM_MAX_N) { std::snprintf(g_err, sizeof(g_err), "PERM N > %d", ROSEN_PERM_MAX_N); return ROSEN_ERANGE; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* sc = nullptr;
+    int rc = get_scratch(&sc);
+    if (rc) return rc;
+    const Sizes zs = output_sizes(N, n_tours, sizeof(int32_t));
+    Staging st;
+    if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_tours * sizeof(rosen::ChainRecord)))) return rc;
+        if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
+        if (!sc->perm_thr) CK(cudaMalloc(&sc->perm_thr, sizeof(double) * 2 * (ROSEN_PERM_MAX_N + 1)));
+    }
+    CK(cudaMemcpyAsync(sc->perm_thr, ln_lo, sizeof(double) * (size_t)(N + 1), cudaMemcpyHostToDevice, stream));
+    CK(cudaMemcpyAsync(sc->perm_thr + ROSEN_PERM_MAX_N + 1, ln_hi, sizeof(double) * (size_t)(N + 1), cudaMemcpyHostToDevice, stream));
+    CK(cudaMemsetAsync(sc->hash_ticket, 0, sizeof(unsigned long long), stream));
+    rosen::PermParams pp{};
+    pp.N = N; pp.n_tours = n_tours; pp.tour_offset = tour_offset;
+    pp.key0 = (uint32_t)seed; pp.key1 = (uint32_t)(seed >> 32);
+    pp.ln_lo = sc->perm_thr; pp.ln_hi = sc->perm_thr + ROSEN_PERM_MAX_N + 1; pp.ln_ref = ln_ref; pp.max_nodes = max_nodes;
+    pp.out = st.dev; pp.partials = sc->dev;
+    rosen::partition_chains(n_tours, &pp.chunk, &pp.n_vblocks, 256u);
+    pp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
+    pp.lmax = sc->lmax; pp.ticket = sc->hash_ticket;
+    rc = rosen::launch_lattice_perm(pp, stream, &g_kernel);
+    if (rc < 0) return fail_cuda(cudaGetLastError(), "PERM kernel launch");
+    g_launches += rc;
+    return finish(sc, (int)pp.n_vblocks, n_tours, 0.0, pp.lmax + rosen::kMaxPartials, outputs, zs, st, summary, nullptr, stream);
+}
+
 }  // namespace
 
 extern "C" {
@@ -493,6 +536,12 @@ int rosen_realspace_generate_model(int32_t N, uint64_t n_chains, int32_t k_trial
                                    const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
 {
     return realspace_model_impl(N, n_chains, k_trials, bond_len, sigma, lambda, beta_eps, seed, chain_offset, outputs, summary, cuda_stream);
+}
+
+int rosen_lattice_perm(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset, const double* ln_lo, const double* ln_hi,
+                       double ln_ref, uint32_t max_nodes, const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream)
+{
+    return perm_impl(N, n_tours, seed, tour_offset, ln_lo, ln_hi, ln_ref, max_nodes, outputs, summary, cuda_stream);
 }
 
 int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged)
@@ -613,6 +662,7 @@ int rosen_workspace_release(void)
     if (s.hash_tables) { cudaFree(s.hash_tables); s.hash_tables = nullptr; s.hash_tables_bytes = 0; }
     if (s.hash_rec) { cudaFree(s.hash_rec); s.hash_rec = nullptr; s.hash_rec_bytes = 0; }
     if (s.hash_ticket) { cudaFree(s.hash_ticket); s.hash_ticket = nullptr; }
+    if (s.perm_thr) { cudaFree(s.perm_thr); s.perm_thr = nullptr; }
     return ROSEN_OK;
 }
 int32_t rosen_last_launch_count(void) { return g_launches; }

@@ -96,6 +96,25 @@ struct ModelParams {
     double*    lmax;            // [kMaxPartials + 1] scratch of the max pass
 };
 
+// PERM (lattice_perm.cu): one record per tour, thresholds in device memory.
+struct PermParams {
+    int32_t    N;
+    uint64_t   n_tours;
+    uint64_t   tour_offset;
+    uint32_t   key0, key1;
+    const double* ln_lo;        // [N + 1] device copies of the caller's thresholds (index = number of monomers)
+    const double* ln_hi;
+    double     ln_ref;          // reference of the leaf weights inside a tour: w = exp(lnW - ln_ref)
+    uint32_t   max_nodes;
+    DevOutputs out;
+    Partial*   partials;
+    uint32_t   chunk;
+    uint32_t   n_vblocks;
+    ChainRecord* rec;           // [n_tours]; alive bit 0 = the tour has a leaf, bit 1 = stopped at max_nodes
+    double*    lmax;
+    unsigned long long* ticket; // zeroed before the launch
+};
+
 constexpr uint32_t kRealLongCandCap = 160;
 
 // Long-chain real-space path (realspace_long.cu): one warp grows one chain; chain, cell table and cell lists in HBM.
@@ -157,6 +176,8 @@ int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t str
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 // lattice_model.cu: generation kernel + record reduction (max pass included); returns the launches made
 int launch_lattice_model(const ModelParams& p, cudaStream_t stream, const char** kernel_name);
+// lattice_perm.cu: tour kernel + record reduction; returns the launches made
+int launch_lattice_perm(const PermParams& p, cudaStream_t stream, const char** kernel_name);
 // realspace.cu: the direction map of DESIGN.md 3.3 alone, out[3 i ..] = direction(wz[i], wphi[i]) (device pointers)
 int launch_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* out, cudaStream_t stream);
 int launch_finalize(const Partial* partials, int n_partials, uint64_t n_chains, double ln_shift, const double* ln_shift_dev,

@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(256) records_max_kernel(const ChainRecord* __r
     for (uint32_t it = 0; it < chunk / 256u; ++it) {
         const uint64_t idx = (uint64_t)blockIdx.x * chunk + (uint64_t)it * 256u + threadIdx.x;
         if (idx >= n_chains) break;
-        if (rec[idx].alive != 0u) v = fmax(v, rec[idx].lnW);
+        if ((rec[idx].alive & 1u) != 0u) v = fmax(v, rec[idx].lnW);
     }
     for (int d = 16; d >= 1; d >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, d));
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
@@ -283,13 +283,13 @@ __global__ void __launch_bounds__(256) reduce_records_kernel(const ChainRecord* 
         const uint64_t idx = (uint64_t)vb * chunk + (uint64_t)it * 256u + threadIdx.x;
         if (idx >= n_chains) break;
         const ChainRecord r = rec[idx];
-        const bool alive = r.alive != 0u;
+        const bool alive = (r.alive & 1u) != 0u;                       // bit 1 (PERM): tour stopped at max_nodes, reported as 2
         const double wgt = alive ? exp(r.lnW - ln_shift) : 0.0;
         acc.sum_w += wgt; acc.sum_w_ree2 += wgt * r.ree2; acc.sum_w_rg2 += wgt * r.rg2; acc.sum_w2 += wgt * wgt;
         acc.n_dead += alive ? 0u : 1u; acc.n_steps += r.steps;
         if (out.digest) { acc.digest_xor ^= r.digest; acc.digest_sum += r.digest; out.digest[idx] = r.digest; }
         if (out.lnW) out.lnW[idx] = r.lnW;
-        if (out.alive) out.alive[idx] = alive ? 1 : 0;
+        if (out.alive) out.alive[idx] = (r.alive & 2u) ? 2 : (alive ? 1 : 0);
         if (out.ree2) out.ree2[idx] = r.ree2;
         if (out.rg2) out.rg2[idx] = r.rg2;
     }
