@@ -62,22 +62,41 @@ def algorithmic_thread_instr(w: workloads.Workload) -> float:
     return 7.0 * (N - 1) * (N - 2) / 2.0 + (N - 1) * (7.0 * 3.2 * k + 35.0 * k + 45.0 * k + 30.0)
 
 
-def profile_traffic(w: workloads.Workload):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed ncu summary of
-    this workload (profiles/), per launch; None if no capture is committed."""
-    name = {"lattice_N64_2p24": "r01d_lattice_cfg2.md", "realspace_N64_k16_2p22": "r01d_realspace_cfg3.md",
-            "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md",
-            "realspace_long_N4096_k16_2p16": "r01e_realspace_long_N4096.md"}.get(w.name)
+PROFILE_OF = {   # committed ncu summary (profiles/) of the dominant kernel of each workload
+    "lattice_N16_2p16": "r02_lattice_cfg1.md", "lattice_N64_2p24": "r02_lattice_cfg2.md",
+    "realspace_N64_k16_2p22": "r02_realspace_cfg3.md", "realspace_N256_k64_2p20_dump": "r02_realspace_cfg5.md",
+    "lattice_sweep_N128_2p24": "r02_lattice_sweep_N128.md", "lattice_sweep_N256_2p24": "r02_lattice_sweep_N256.md",
+    "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md", "realspace_long_N4096_k16_2p16": "r01e_realspace_long_N4096.md",
+}
+
+
+def profile_metrics(w: workloads.Workload) -> dict:
+    """Per-launch metrics of the dominant kernel from the committed ncu summary of this workload (profiles/): DRAM traffic,
+    warp-instructions executed, threads per instruction, issue-active %. Empty if no capture is committed."""
+    name = PROFILE_OF.get(w.name)
     path = os.path.join(ROOT, "profiles", name) if name else None
     if not path or not os.path.exists(path):
-        return None
+        return {}
     mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
-    total = 0.0
+    out = {"file": "profiles/" + name}
+    traffic = None
     for line in open(path):
         cells = [c.strip() for c in line.split("|")]
-        if len(cells) >= 4 and cells[1] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
-            total += float(cells[3]) * mult.get(cells[2], 1.0)
-    return total
+        if len(cells) < 4:
+            continue
+        try:
+            if cells[1] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                traffic = (traffic or 0.0) + float(cells[3]) * mult.get(cells[2], 1.0)
+            elif cells[1] == "smsp__inst_executed.sum":
+                out["warp_inst_executed"] = float(cells[3])
+            elif cells[1] == "smsp__thread_inst_executed_per_inst_executed.ratio":
+                out["active_lane_ratio"] = float(cells[3])
+            elif cells[1] == "smsp__issue_active.avg.pct_of_peak_sustained_active":
+                out["issue_active_pct"] = float(cells[3])
+        except ValueError:
+            continue
+    out["traffic"] = traffic
+    return out
 
 
 def load_measured_peaks():
@@ -157,6 +176,23 @@ def make_calls(R, torch, w: workloads.Workload, offset: int, stream):
                 "lnW": torch.empty((w.n_chains,), dtype=torch.float64, device="cuda")}
     d2h = R.SUMMARY_BYTES + sum(t.numel() * t.element_size() for t in dump.values())
 
+    if w.perm is not None or w.beta_eps is not None:
+        # model / PERM calls have no _async twin: the device-timed leg enqueues the call without a
+        # host summary (no synchronisation), the end-to-end leg takes the summary
+        if w.perm is not None:
+            lo, hi, ref = workloads.perm_thresholds(w.N, *w.perm)
+
+            def call(summary):
+                return R.rosen_lattice_perm(w.N, w.n_chains, w.seed, lo, hi, ref, tour_offset=offset, stream=stream, summary=summary)[0]
+        elif w.kind == "lattice":
+            def call(summary):
+                return R.rosen_lattice_generate_model(w.N, w.n_chains, w.seed, z=w.z, beta_eps=w.beta_eps, chain_offset=offset,
+                                                      stream=stream, summary=summary)[0]
+        else:
+            def call(summary):
+                return R.rosen_realspace_generate_model(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.lam, w.beta_eps, w.seed,
+                                                        chain_offset=offset, stream=stream, summary=summary)[0]
+        return (lambda summary_device: call(False)), (lambda: call(True)), d2h
     if w.kind == "lattice":
         def enqueue(summary_device):
             R.rosen_lattice_generate_async(w.N, w.n_chains, w.seed, offset, outputs=dump,
@@ -180,6 +216,14 @@ def make_calls(R, torch, w: workloads.Workload, offset: int, stream):
 
 def oracle_call(w: workloads.Workload, n_chains: int, offset: int = 0):
     import oracle  # test infrastructure; allowed here for cpu_baseline / --impl reference only
+    if w.perm is not None:
+        lo, hi, ref = workloads.perm_thresholds(w.N, *w.perm)
+        return oracle.lattice_perm(w.N, n_chains, w.seed, lo, hi, ref, tour_offset=offset, outputs=())
+    if w.beta_eps is not None and w.kind == "lattice":
+        return oracle.lattice_model_generate(w.N, n_chains, w.seed, z=w.z, beta_eps=w.beta_eps, chain_offset=offset, outputs=())
+    if w.beta_eps is not None:
+        return oracle.realspace_model_generate(w.N, n_chains, w.k_trials, w.bond_len, w.sigma, w.lam, w.beta_eps, w.seed,
+                                               chain_offset=offset, outputs=())
     if w.kind == "lattice":
         return oracle.lattice_generate(w.N, n_chains, w.seed, chain_offset=offset, outputs=())
     return oracle.realspace_generate(w.N, n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, chain_offset=offset,
@@ -286,13 +330,18 @@ def run_product(args, w, rank, world, local_rank):
     t1 = time.perf_counter()
     clocks = sampler.stop(t0, t1)
     total_ms = sum(ms)
-    summary = R.summary_from_device(summary_dev)
+    extra = w.perm is not None or w.beta_eps is not None
+    summary = sync_call() if extra else R.summary_from_device(summary_dev)
 
     # ---- dominant kernel alone (generation kernel, no second pass), live, same stream ------------
     timed(lambda: enqueue(None), 2)
     kms = timed(lambda: enqueue(None), max(3, min(steps, 10)))
     kernel_ms = sum(kms) / len(kms)
 
+    dump_probe_conf = dump_probe_lnw = None
+    if w.dump and w.kind == "realspace":
+        dump_probe_conf = torch.empty((w.n_chains, w.N, 3), dtype=torch.float32, device="cuda")
+        dump_probe_lnw = torch.empty((w.n_chains,), dtype=torch.float64, device="cuda")
     # ---- dump path (config 5): store phase D1 in situ = time(generation + dump) - time(generation only), same
     # launch geometry and lane mapping; bytes stored / that difference = achieved HBM write GB/s of the store phase
     dump_info = None
@@ -306,7 +355,13 @@ def run_product(args, w, rank, world, local_rank):
         nbytes = w.n_chains * (12 * w.N + 8)
         diff = t_all - t_gen
         resolved = diff > 0.01 * t_all          # below 1 % of the call the difference is timing noise
+        # the store phase alone: the same store routine, block size and grid over a resident synthetic chain (rosen_realspace_dump_probe)
+        def probe():
+            R.rosen_realspace_dump_probe(w.N, w.n_chains, dump_probe_conf, dump_probe_lnw, stream=stream)
+        timed(probe, 2)
+        t_probe = min(timed(probe, 5))
         dump_info = {"bytes_per_step": nbytes, "with_dump_ms": t_all, "generation_only_ms": t_gen, "store_phase_ms": diff,
+                     "isolated_store_ms": t_probe, "isolated_store_GBps": nbytes / (t_probe * 1e-3) / 1e9,
                      "achieved_GBps": nbytes / (diff * 1e-3) / 1e9 if resolved else None,
                      "whole_call_GBps": nbytes / (t_all * 1e-3) / 1e9,
                      "note": None if resolved else "store phase not resolvable: hidden under generation (compute-bound call)"}
@@ -344,7 +399,7 @@ def run_product(args, w, rank, world, local_rank):
     peak_winst = n_sm * 4 * sm_hz                           # 4 schedulers/SM, 1 warp-instruction/clk each
     alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
     achieved = alg_winst / (kernel_ms * 1e-3)
-    if w.kind == "lattice" and w.N >= 193:
+    if w.kind == "lattice" and w.N >= 193 and not extra:
         # hash-map kernel (DESIGN.md 5.5 / 6): ncu shows it issue-bound (60.5 % issue-active, 28 % of DRAM peak), so the
         # roofline is the issue peak; algorithmic work per ATTEMPTED step (not per nominal step: most long chains die
         # early): 3 cube look-ups (hash 8 + compare 6 each), 6 occupancy bits (4 each), count/choose 15, insert 10,
@@ -358,11 +413,14 @@ def run_product(args, w, rank, world, local_rank):
         real_long_instr = w.k_trials * (80.0 + 7.0 * 3.2) + 27 * 14.0 + 40 * 10.0 + 50.0
         alg_winst = real_long_instr * (steps_attempted / world) / 32.0
         achieved = alg_winst / (kernel_ms * 1e-3)
+    prof = profile_metrics(w)
+    if extra:
+        achieved = float("nan")
     roofline = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s",
-                "frac": achieved / peak_winst, "traffic": profile_traffic(w), "kernel": kernel_name, "kernel_ms": kernel_ms,
+                "frac": achieved / peak_winst, "traffic": prof.get("traffic"), "kernel": kernel_name, "kernel_ms": kernel_ms,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
                 "algorithmic_thread_instr_per_chain": algorithmic_thread_instr(w)}
-    if w.kind == "lattice" and w.N >= 193:
+    if w.kind == "lattice" and w.N >= 193 and not extra:
         del roofline["algorithmic_thread_instr_per_chain"]
         roofline["algorithmic_thread_instr_per_attempted_step"] = HASH_INSTR_PER_STEP
         roofline["note"] = "kernel_ms covers table memset + generation kernel + record reduction"
@@ -372,6 +430,21 @@ def run_product(args, w, rank, world, local_rank):
         roofline["note"] = "kernel_ms covers workspace memset + generation kernel + record reduction"
     if clocks.get("sm_mhz"):
         roofline["frac_at_measured_clock"] = achieved / (n_sm * 4 * clocks["sm_mhz"] * 1e6)
+    if extra:
+        roofline = {"bound": "alu", "achieved": None, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s", "frac": None, "traffic": None,
+                    "kernel": kernel_name, "kernel_ms": kernel_ms,
+                    "note": "model / PERM workload (SURVEY.md 8(f) rows 4, 2): timed, no algorithmic-work model stated"}
+    if w.kind == "lattice" and w.N < 193 and not extra:
+        # SURVEY.md 8(d) wrote "930 x ~5" per site test where DESIGN.md 6 counts the 6 equality tests of the method: both
+        survey = 5.0 * lattice_site_tests(w.N) + 70.0 * ((w.N + 3) // 4) + 20.0 * (w.N - 1)
+        roofline["frac_survey_coefficient"] = survey * w.n_chains / 32.0 / (kernel_ms * 1e-3) / peak_winst
+        roofline["algorithmic_thread_instr_per_chain_survey"] = survey
+    if prof.get("warp_inst_executed"):
+        # "utilisation is not usefulness": what the kernel ISSUES per attempted step next to what the method needs
+        roofline["issued_thread_instr_per_attempted_step"] = prof["warp_inst_executed"] * 32.0 / (steps_attempted / world)
+        roofline["active_lane_ratio"] = prof.get("active_lane_ratio")
+        roofline["issue_active_pct_ncu"] = prof.get("issue_active_pct")
+        roofline["profile"] = prof.get("file")
 
     out = {
         "metric": METRIC, "value": value, "unit": "chains/s", "n_gpus": world, "steps": steps, "warmup": warmup,
@@ -394,12 +467,21 @@ def run_product(args, w, rank, world, local_rank):
     if dump_info is not None:
         dump_info["peak_GBps"] = float(peaks.get("hbm_gbs", 6650.0))
         dump_info["frac"] = dump_info["achieved_GBps"] / dump_info["peak_GBps"] if dump_info["achieved_GBps"] else None
+        dump_info["isolated_store_frac"] = dump_info["isolated_store_GBps"] / dump_info["peak_GBps"]
         out["dump_path"] = dump_info
     if world == 1 and not args.no_cpu_baseline:
         m, dt, _ = time_oracle(w, args.cpu_seconds / 2)
         cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
         per = max(16 if w.N <= 2048 else 1, int(m / dt * args.cpu_seconds / 2))   # ~cpu_seconds/2 of work per thread
         ma, dta = time_oracle_all_cores(w, per, cores)
+        if w.kind == "realspace" and not extra:
+            # decision parity on the single-thread sample: chains whose digest differs from the oracle's = flip fraction
+            import numpy as np
+            import oracle
+            ref = oracle.realspace_generate(w.N, m, w.k_trials, w.bond_len, w.sigma, w.seed, chain_offset=offset, outputs=("digest",))
+            _, tg = R.rosen_realspace_generate(w.N, m, w.k_trials, w.bond_len, w.sigma, w.seed, chain_offset=offset, outputs=("digest",))
+            out["flip_fraction"] = {"value": float((tg["digest"].cpu().numpy().view(np.uint64) != ref.digest).mean()),
+                                    "chains": m, "bar": 1e-4}
         out["cpu_baseline"] = {"value": ma / dta, "unit": "chains/s", "cores": cores, "kind": "oracle",
                                "sample": f"{cores} threads x {per} chains (disjoint chain-id ranges of {w.name}), {dta:.1f} s",
                                "single_thread": {"value": m / dt, "cores": 1,

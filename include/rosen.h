@@ -212,6 +212,15 @@ ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trial
  * part with sum_w > 0. Returns ROSEN_EINVAL if count == 0 or a shift is not finite.
  * Pure host function.
  */
+/*
+ * The store phase of rosen_realspace_dump ALONE ("HBM GB/s is only meaningful for the store phase
+ * measured alone ... a dump-only kernel"): every lane group keeps one synthetic chain (r_i = (i, i/2, -i)) resident in
+ * shared memory and stores it to conf[c][N][3] (and (double)c to lnW[c], if non-NULL) for every chain c < n_chains, with
+ * the store routine, block size and grid of the config-5 kernel realspace_kernel<G=32>. Enqueue only; conf, lnW are
+ * DEVICE pointers of 3 N n_chains floats / n_chains doubles. A measurement entry: bytes stored = n_chains (12 N + 8).
+ */
+ROSEN_API int rosen_realspace_dump_probe(int32_t N, uint64_t n_chains, float* conf, double* lnW, void* cuda_stream);
+
 ROSEN_API int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged);
 
 /*

@@ -92,6 +92,8 @@ def load_library() -> C.CDLL:
     L.rosen_lattice_perm.argtypes = [i32, u64, u64, u64, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, C.c_uint32,
                                      C.POINTER(rosen_outputs), C.POINTER(rosen_summary), vp]
     L.rosen_lattice_perm.restype = C.c_int
+    L.rosen_realspace_dump_probe.argtypes = [i32, u64, vp, vp, vp]
+    L.rosen_realspace_dump_probe.restype = C.c_int
     L.rosen_direction_eval.argtypes = [vp, vp, u64, vp, i32, vp]
     L.rosen_direction_eval.restype = C.c_int
     L.rosen_workspace_bytes.argtypes = []
@@ -193,7 +195,7 @@ def rosen_realspace_generate(N: int, n_chains: int, k_trials: int, bond_len: flo
 
 
 def rosen_lattice_generate_model(N: int, n_chains: int, seed: int, z: int = 6, beta_eps: float = 0.0, chain_offset: int = 0,
-                                 outputs: Iterable[str] = (), stream=None, host_outputs: bool = False):
+                                 outputs: Iterable[str] = (), stream=None, host_outputs: bool = False, summary: bool = True):
     """rosen_lattice_generate_model of include/rosen.h (z = 6 / 26 trial set, contact energy). Returns (summary, tensors)."""
     L = load_library()
     torch = _torch()
@@ -201,13 +203,14 @@ def rosen_lattice_generate_model(N: int, n_chains: int, seed: int, z: int = 6, b
         raise RosenError(ROSEN_ECUDA, "no CUDA device (there is no CPU fallback)")
     tensors, st = _alloc_outputs(N, n_chains, "int32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
     s = rosen_summary()
-    _check(L.rosen_lattice_generate_model(N, n_chains, seed, chain_offset, z, beta_eps, C.byref(st), C.byref(s), _stream_ptr(stream)))
-    return s.as_dict(), tensors
+    _check(L.rosen_lattice_generate_model(N, n_chains, seed, chain_offset, z, beta_eps, C.byref(st),
+                                          C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), tensors
 
 
 def rosen_realspace_generate_model(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, lam: float,
                                    beta_eps: float, seed: int, chain_offset: int = 0, outputs: Iterable[str] = (),
-                                   stream=None, host_outputs: bool = False):
+                                   stream=None, host_outputs: bool = False, summary: bool = True):
     """rosen_realspace_generate_model of include/rosen.h (square well of range lam * sigma). Returns (summary, tensors)."""
     L = load_library()
     torch = _torch()
@@ -216,12 +219,13 @@ def rosen_realspace_generate_model(N: int, n_chains: int, k_trials: int, bond_le
     tensors, st = _alloc_outputs(N, n_chains, "float32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
     s = rosen_summary()
     _check(L.rosen_realspace_generate_model(N, n_chains, k_trials, bond_len, sigma, lam, beta_eps, seed, chain_offset,
-                                            C.byref(st), C.byref(s), _stream_ptr(stream)))
-    return s.as_dict(), tensors
+                                            C.byref(st), C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), tensors
 
 
 def rosen_lattice_perm(N: int, n_tours: int, seed: int, ln_lo, ln_hi, ln_ref: float, max_nodes: int = 1 << 20,
-                       tour_offset: int = 0, outputs: Iterable[str] = (), stream=None, host_outputs: bool = False):
+                       tour_offset: int = 0, outputs: Iterable[str] = (), stream=None, host_outputs: bool = False,
+                       summary: bool = True):
     """rosen_lattice_perm of include/rosen.h: ln_lo, ln_hi = sequences of N+1 floats. Returns (summary, tensors)."""
     L = load_library()
     torch = _torch()
@@ -232,8 +236,9 @@ def rosen_lattice_perm(N: int, n_tours: int, seed: int, ln_lo, ln_hi, ln_ref: fl
     lo = (C.c_double * (N + 1))(*[float(v) for v in ln_lo]); hi = (C.c_double * (N + 1))(*[float(v) for v in ln_hi])
     tensors, st = _alloc_outputs(N, n_tours, "int32", outputs, torch.device("cuda", torch.cuda.current_device()), host_outputs)
     s = rosen_summary()
-    _check(L.rosen_lattice_perm(N, n_tours, seed, tour_offset, lo, hi, ln_ref, max_nodes, C.byref(st), C.byref(s), _stream_ptr(stream)))
-    return s.as_dict(), tensors
+    _check(L.rosen_lattice_perm(N, n_tours, seed, tour_offset, lo, hi, ln_ref, max_nodes, C.byref(st),
+                                C.byref(s) if summary else None, _stream_ptr(stream)))
+    return (s.as_dict() if summary else None), tensors
 
 
 SUMMARY_BYTES = C.sizeof(rosen_summary)
@@ -319,6 +324,12 @@ def rosen_fit_exponents(N, mean_ree2, ln_mean_W, use_steps: bool = True) -> Dict
     _check(L.rosen_fit_exponents((C.c_int32 * n)(*[int(v) for v in N]), (C.c_double * n)(*[float(v) for v in mean_ree2]),
                                  (C.c_double * n)(*[float(v) for v in ln_mean_W]), n, 1 if use_steps else 0, C.byref(out)))
     return {name: getattr(out, name) for name, _ in out._fields_}
+
+
+def rosen_realspace_dump_probe(N: int, n_chains: int, conf, lnW=None, stream=None) -> None:
+    """rosen_realspace_dump_probe: conf = float32 CUDA tensor [n_chains, N, 3], lnW = float64 CUDA tensor [n_chains] or None."""
+    _check(load_library().rosen_realspace_dump_probe(N, n_chains, conf.data_ptr(), lnW.data_ptr() if lnW is not None else None,
+                                                     _stream_ptr(stream)))
 
 
 def rosen_direction_eval(wz, wphi, stream=None):

@@ -612,6 +612,19 @@ int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double*
     return ROSEN_OK;
 }
 
+int rosen_realspace_dump_probe(int32_t N, uint64_t n_chains, float* conf, double* lnW, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "dump_probe_kernel<G=32>";
+    if (N < 2 || N > ROSEN_REALSPACE_SCAN_MAX_N || n_chains == 0 || !conf) {
+        std::snprintf(g_err, sizeof(g_err), "need 2 <= N <= %d, n_chains >= 1 and a device conf buffer", ROSEN_REALSPACE_SCAN_MAX_N);
+        return ROSEN_EINVAL;
+    }
+    if (rosen::launch_dump_probe(N, n_chains, conf, lnW, static_cast<cudaStream_t>(cuda_stream)) < 0)
+        return fail_cuda(cudaGetLastError(), "dump_probe_kernel");
+    g_launches = 1;
+    return ROSEN_OK;
+}
+
 int rosen_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, float* dir_xyz, int32_t memory, void* cuda_stream)
 {
     g_err[0] = 0; g_launches = 0; g_kernel = "direction_eval_kernel";

@@ -174,6 +174,8 @@ int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t ch
 int real_long_max_warps(int k, int* warps_out);
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
+// realspace.cu: the D1 store phase alone over a resident synthetic chain (measurement entry rosen_realspace_dump_probe)
+int launch_dump_probe(int N, uint64_t n_chains, float* conf, double* lnW, cudaStream_t stream);
 // lattice_model.cu: generation kernel + record reduction (max pass included); returns the launches made
 int launch_lattice_model(const ModelParams& p, cudaStream_t stream, const char** kernel_name);
 // lattice_perm.cu: tour kernel + record reduction; returns the launches made

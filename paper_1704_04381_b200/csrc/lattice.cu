@@ -207,7 +207,9 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
         Partial acc = partial_zero();
         for (uint32_t it = 0; it < per_thread; ++it) {
             const uint64_t idx = (uint64_t)vb * p.chunk + (uint64_t)it * blockDim.x + threadIdx.x;
-            if (idx >= p.n_chains) break;
+            const bool active = idx < p.n_chains;
+            if (TRAJ) { if (!__any_sync(0xffffffffu, active)) break; }    // the conformation store below is warp-cooperative:
+            else if (!active) break;                                     // lanes past the end grow a chain nobody keeps
             const uint64_t chain = p.chain_offset + idx;
             const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
 
@@ -220,7 +222,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
             uint32_t hist = 0, dead = 0;     // dead = step of the first m = 0 (0: alive)
             double lnW_w = 0.0;             // RUNSUM: running sum in step order
             uint64_t dg = 0xCBF29CE484222325ull;
-            uint8_t* mrow = TRAJ && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
+            uint8_t* mrow = TRAJ && active && p.out.m_seq ? p.out.m_seq + idx * (uint64_t)(N - 1) : nullptr;
 
 #pragma unroll 2
             for (int q = 0; 4 * q < N; ++q) {
@@ -285,25 +287,37 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                 rg2 = (double)num / ((double)N * (double)N);
             }
             const double wgt = alive ? exp(lnW - p.ln_shift) : 0.0;
-            acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
-            acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
-            if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
+            if (!TRAJ || active) {
+                acc.sum_w += wgt; acc.sum_w_ree2 += wgt * ree2; acc.sum_w_rg2 += wgt * rg2; acc.sum_w2 += wgt * wgt;
+                acc.n_dead += alive ? 0u : 1u; acc.n_steps += steps;
+                if (DIGEST) { acc.digest_xor ^= dg; acc.digest_sum += dg; }
 
-            if (p.out.lnW) p.out.lnW[idx] = lnW;
-            if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
-            if (p.out.ree2) p.out.ree2[idx] = ree2;
-            if (p.out.rg2) p.out.rg2[idx] = rg2;
-            if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
+                if (p.out.lnW) p.out.lnW[idx] = lnW;
+                if (p.out.alive) p.out.alive[idx] = alive ? 1 : 0;
+                if (p.out.ree2) p.out.ree2[idx] = ree2;
+                if (p.out.rg2) p.out.rg2[idx] = rg2;
+                if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
+            }
             if (TRAJ && p.out.conf) {
-                int32_t* c = reinterpret_cast<int32_t*>(p.out.conf) + idx * (uint64_t)N * 3;
-                const int placed = alive ? N : (int)steps;
-                for (int i = 0; i < N; ++i) {
-                    const uint32_t v = ((i & 1) ? od : ev)[i >> 1];
-                    const bool ok = i < placed;
-                    c[3 * i + 0] = ok ? (int)(v & kFieldMask) - kBias : 0;
-                    c[3 * i + 1] = ok ? (int)((v >> B) & kFieldMask) - kBias : 0;
-                    c[3 * i + 2] = ok ? (int)((v >> (2 * B)) & kFieldMask) - kBias : 0;
+                // D1: the warp stores its 32 chains one after the other, consecutive lanes writing consecutive int32 of the
+                // chain's [N][3] row block (128 contiguous bytes per instruction); zeros from the death step on.
+                __syncwarp();
+                const int lane = threadIdx.x & 31;
+                const int my_placed = active ? (alive ? N : (int)steps) : -1;
+                const uint32_t* wbase = chains + (size_t)(threadIdx.x - lane) * stride;
+                for (int L = 0; L < 32; ++L) {
+                    const int placed = __shfl_sync(0xffffffffu, my_placed, L);
+                    if (placed < 0) continue;                                  // warp-uniform
+                    const uint32_t* cev = wbase + (size_t)L * stride;
+                    const uint32_t* cod = cev + half4;
+                    int32_t* c = reinterpret_cast<int32_t*>(p.out.conf) + (idx - lane + L) * (uint64_t)N * 3;
+                    for (int e = lane; e < 3 * N; e += 32) {
+                        const int i = (int)(((uint32_t)e * 43691u) >> 17), a = e - 3 * i;      // e / 3, e % 3 (e < 98304)
+                        const uint32_t v = ((i & 1) ? cod : cev)[i >> 1];
+                        c[e] = i < placed ? (int)((v >> (B * a)) & kFieldMask) - kBias : 0;
+                    }
                 }
+                __syncwarp();
             }
         }
         block_reduce_store(acc, scratch, p.partials + vb);

@@ -105,6 +105,51 @@ __device__ __forceinline__ uint32_t candidate_bits(const float4* base, int cnt, 
     }
 }
 
+// D1 store phase ("flushed to the global memory"): the group's lanes stream the chain out of shared memory,
+// float4 (x, y, z, -) -> crow[N][3], zeros from monomer `placed` on. Rows are 12 N bytes: 16-byte aligned when N is a
+// multiple of 4, then consecutive lanes store consecutive 16-byte pieces (G = 32: 512 contiguous bytes per instruction);
+// otherwise 4-byte stores, still consecutive across lanes.
+template <int G>
+__device__ __forceinline__ void store_conf(const float4* R4, float* crow, int N, int placed, int gl)
+{
+    const float* Rf = reinterpret_cast<const float*>(R4);
+    if ((N & 3) == 0) {
+        float4* c4 = reinterpret_cast<float4*>(crow);
+        for (int v = gl; v < 3 * (N >> 2); v += G) {
+            float o[4];
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+                const uint32_t e = 4u * (uint32_t)v + cc, i = (e * 43691u) >> 17;       // e / 3 for e < 98304
+                o[cc] = (int)i < placed ? Rf[e + i] : 0.0f;                                // word 4 i + (e - 3 i)
+            }
+            c4[v] = make_float4(o[0], o[1], o[2], o[3]);
+        }
+    } else {
+        for (int e = gl; e < 3 * N; e += G) {
+            const uint32_t i = ((uint32_t)e * 43691u) >> 17;
+            crow[e] = (int)i < placed ? Rf[e + i] : 0.0f;
+        }
+    }
+}
+
+// The store phase alone (rosen_realspace_dump_probe; SURVEY.md 8(d) "isolated store phase ... a dump-only kernel"): every
+// group keeps one synthetic chain resident in shared memory and stores it, with store_conf above and the launch geometry
+// of realspace_kernel<G, ...>, once per chain id of the call (+ one fp64 per chain, like lnW).
+template <int G>
+__global__ void __launch_bounds__(256, 3) dump_probe_kernel(int N, uint64_t n_chains, float* conf, double* lnW)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int gl = threadIdx.x & (G - 1);
+    const uint32_t group = threadIdx.x / G, gpb = blockDim.x / G;
+    float4* R4 = reinterpret_cast<float4*>(smem_raw + group_bytes(N, G, false) * group);
+    for (int i = gl; i < N; i += G) R4[i] = make_float4((float)i, 0.5f * (float)i, -(float)i, 0.f);
+    __syncwarp();
+    for (uint64_t idx = (uint64_t)blockIdx.x * gpb + group; idx < n_chains; idx += (uint64_t)gridDim.x * gpb) {
+        store_conf<G>(R4, conf + idx * (uint64_t)N * 3, N, N, gl);
+        if (gl == 0 && lnW) lnW[idx] = (double)idx;
+    }
+}
+
 // MSEQ: the per-step m sequence is requested (one shared-memory byte per step). The conformation dump needs no
 // variant: the chain is in shared memory anyway and is stored once, after the last step, if p.out.conf is set.
 // WELL: square-well model of DESIGN.md 3.6 (rosen_realspace_generate_model): contacts inside lambda sigma are counted
@@ -340,31 +385,9 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             if (p.out.rg2) p.out.rg2[idx] = rg2;
             if (DIGEST && p.out.digest) p.out.digest[idx] = dg;
         }
-        // ---- D1: the group streams its chain out of shared memory, float4 (x, y, z, -) -> [N][3], zeros from the
-        // death step on. Rows are 12 N bytes: 16-byte aligned when N is a multiple of 4, then consecutive lanes store
-        // consecutive 16-byte pieces (G = 32: 512 contiguous bytes per instruction); otherwise 4-byte stores.
-        if (p.out.conf != nullptr && active) {
-            const int placed = alive ? N : (int)steps;
-            const float* Rf = reinterpret_cast<const float*>(R4);
-            float* crow = reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3;
-            if ((N & 3) == 0) {
-                float4* c4 = reinterpret_cast<float4*>(crow);
-                for (int v = gl; v < 3 * (N >> 2); v += G) {
-                    float o[4];
-#pragma unroll
-                    for (int cc = 0; cc < 4; ++cc) {
-                        const uint32_t e = 4u * (uint32_t)v + cc, i = (e * 43691u) >> 17;       // e / 3 for e < 98304
-                        o[cc] = (int)i < placed ? Rf[e + i] : 0.0f;                                // word 4 i + (e - 3 i)
-                    }
-                    c4[v] = make_float4(o[0], o[1], o[2], o[3]);
-                }
-            } else {
-                for (int e = gl; e < 3 * N; e += G) {
-                    const uint32_t i = ((uint32_t)e * 43691u) >> 17;
-                    crow[e] = (int)i < placed ? Rf[e + i] : 0.0f;
-                }
-            }
-        }
+        // ---- D1
+        if (p.out.conf != nullptr && active)
+            store_conf<G>(R4, reinterpret_cast<float*>(p.out.conf) + idx * (uint64_t)N * 3, N, alive ? N : (int)steps, gl);
         if (MSEQ && active) {
             uint8_t* mr = p.out.m_seq + idx * (uint64_t)(N - 1);
             for (int e = gl; e < N - 1; e += G) mr[e] = mbuf[e];
@@ -439,6 +462,22 @@ int launch_direction_eval(const uint32_t* wz, const uint32_t* wphi, uint64_t n, 
 {
     const uint64_t blocks = (n + 255) / 256;
     direction_eval_kernel<<<(int)(blocks < 4096 ? blocks : 4096), 256, 0, stream>>>(wz, wphi, n, out);
+    return cudaGetLastError() == cudaSuccess ? 1 : -3;
+}
+
+int launch_dump_probe(int N, uint64_t n_chains, float* conf, double* lnW, cudaStream_t stream)
+{
+    constexpr int G = 32;                                    // the geometry of BASELINE config 5 (k = 64: one warp per chain)
+    int dev = 0, n_sm = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    const int threads = block_threads(N, G);
+    const size_t smem = group_bytes(N, G, false) * (threads / G);
+    auto kern = dump_probe_kernel<G>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
+    const uint64_t want = (n_chains + threads / G - 1) / (threads / G), cap = (uint64_t)n_sm * per_sm;
+    kern<<<(int)(want < cap ? want : cap), threads, smem, stream>>>(N, n_chains, conf, lnW);
     return cudaGetLastError() == cudaSuccess ? 1 : -3;
 }
 

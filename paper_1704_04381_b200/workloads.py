@@ -22,6 +22,10 @@ class Workload:
     bond_len: Optional[float] = None
     sigma: Optional[float] = None
     dump: bool = False        # full per-chain conformation output (config 5)
+    z: int = 6                # lattice trial set (model calls: 6 or 26)
+    beta_eps: Optional[float] = None   # contact / well depth in kT: not None selects the model call
+    lam: Optional[float] = None        # real-space well range in units of sigma
+    perm: Optional[Tuple[float, float]] = None   # PERM: thresholds (lo, hi) x the asymptotic c_n
 
     def monomer_steps_nominal(self) -> int:
         return self.n_chains * (self.N - 1)
@@ -47,7 +51,21 @@ LONG_LATTICE = (Workload("lattice_long_N1024_2p20", "lattice", 1024, 1 << 20, 17
 LONG_REALSPACE = (Workload("realspace_long_N4096_k16_2p16", "realspace", 4096, 1 << 16, 17, 16, 1.0, 1.0),
                   Workload("realspace_long_N10000_k64_2p14", "realspace", 10000, 1 << 14, 17, 64, 1.0, 0.8))
 
-CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5, *LONG_LATTICE, *LONG_REALSPACE)}
+# other trial sets / Boltzmann-weighted trials, PERM (n_chains = tours there)
+MODELS = (Workload("lattice_z26_N64_2p20", "lattice", 64, 1 << 20, 19, z=26, beta_eps=0.0),
+          Workload("lattice_z6_contact0.3_N64_2p20", "lattice", 64, 1 << 20, 19, z=6, beta_eps=0.3),
+          Workload("realspace_well1.5_0.4_N64_k16_2p20", "realspace", 64, 1 << 20, 19, 16, 1.0, 1.0, beta_eps=0.4, lam=1.5),
+          Workload("lattice_perm_N256_2p16", "lattice", 256, 1 << 16, 19, perm=(0.5, 2.0)))
+
+CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5, *LONG_LATTICE, *LONG_REALSPACE, *MODELS)}
+
+
+def perm_thresholds(N: int, lo: float, hi: float):
+    """ln_lo, ln_hi [N+1] and ln_ref for PERM: (lo, hi) x the asymptotic form c_n ~ 1.21 mu^n n^(gamma-1), mu = 4.684,
+    gamma = 1.157 (control parameters only: the PERM estimate is unbiased for any thresholds)."""
+    import math
+    ln_c = [0.0, 0.0] + [math.log(1.21) + (n - 1) * math.log(4.684) + 0.157 * math.log(n - 1) for n in range(2, N + 1)]
+    return [v + math.log(lo) for v in ln_c], [v + math.log(hi) for v in ln_c], ln_c[N]
 
 
 def shard(n_chains: int, rank: int, world: int) -> Tuple[int, int]:

@@ -27,7 +27,7 @@ def declared_symbols():
 def test_every_declared_symbol_is_exported(R):
     from paper_1704_04381_b200 import binding
     names = declared_symbols()
-    assert len(names) == 19 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
+    assert len(names) == 20 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
     lib = ctypes.CDLL(binding.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), n
