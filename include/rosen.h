@@ -104,7 +104,8 @@ typedef struct rosen_outputs {
  * word s&3 of Philox4x32-10(key = seed, counter = (id_lo, id_hi, s>>2, 0)). m_s = 0 kills the
  * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N >= ROSEN_LATTICE_HASH_MIN_N the library keeps device
  * workspace (at most 12 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
- * rosen_workspace_release(); the results do not depend on which kernel ran. That workspace is one per device:
+ * rosen_workspace_release(); decisions (trajectory, m sequence, digest) do not depend on which kernel ran, lnW and the sums agree to 1e-12
+ * (different rounding order). The tables are cleared only when they are allocated or their layout changes. That workspace is one per device:
  * long-chain calls (lattice or real space) on the same device must not overlap in time, i.e. enqueue them on one stream
  * or synchronise between streams / host threads.
  */

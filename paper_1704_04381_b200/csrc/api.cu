@@ -38,10 +38,13 @@ struct Scratch {
     void*          hash_tables = nullptr;  size_t hash_tables_bytes = 0;
     void*          hash_rec = nullptr;     size_t hash_rec_bytes = 0;
     unsigned long long* hash_ticket = nullptr;
+    uint32_t*      hash_gen = nullptr;     // [kMaxGenSlots] generation counters of the long-chain kernels' threads / warps
+    uint64_t       ws_layout = 0;          // signature of the table layout the workspace was last cleared for (0: none)
     double*        perm_thr = nullptr;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
 };
 constexpr size_t kHashTableCap = (size_t)12 << 30;  // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
+constexpr size_t kMaxGenSlots = 1 << 20;             // >= resident threads (lattice) / warps (real space) of any device
 Scratch g_scratch[kMaxDevices];
 std::mutex g_mutex;
 
@@ -77,6 +80,20 @@ int grow(void** ptr, size_t* have, size_t need)
     cudaError_t e = cudaMalloc(ptr, need);
     if (e != cudaSuccess) { fail_cuda(e, "cudaMalloc(long-chain workspace)"); *ptr = nullptr; return ROSEN_ENOMEM; }
     *have = need;
+    return ROSEN_OK;
+}
+
+// Long-chain workspace tables are valid across calls as long as their layout (kernel kind, entries per table, number of
+// tables, stride) is the same: every thread / warp keeps its generation counter in hash_gen, so entries of earlier calls
+// read as empty. Only a new allocation or a different layout needs the memset (tables and counters to 0).
+int prepare_workspace(Scratch* sc, uint64_t layout, size_t table_bytes_total, bool reallocated, cudaStream_t stream)
+{
+    if (!sc->hash_gen) CK(cudaMalloc(&sc->hash_gen, kMaxGenSlots * sizeof(uint32_t)));
+    if (sc->ws_layout != layout || reallocated) {
+        CK(cudaMemsetAsync(sc->hash_tables, 0, table_bytes_total, stream));
+        CK(cudaMemsetAsync(sc->hash_gen, 0, kMaxGenSlots * sizeof(uint32_t), stream));
+        sc->ws_layout = layout;
+    }
     return ROSEN_OK;
 }
 
@@ -228,15 +245,19 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
         if (threads > by_mem) threads = by_mem;
         {
             std::lock_guard<std::mutex> lock(g_mutex);
+            const size_t had = sc->hash_tables_bytes;
             if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, threads * table_bytes))) return rc;
             if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
             if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
+            if (threads > kMaxGenSlots) threads = kMaxGenSlots;
+            const uint64_t layout = (1ull << 62) | ((uint64_t)hp.entries << 32) | (uint64_t)threads;
+            if ((rc = prepare_workspace(sc, layout, threads * table_bytes, sc->hash_tables_bytes != had, stream))) return rc;
         }
+        hp.gen_store = sc->hash_gen;
         hp.tables = static_cast<uint64_t*>(sc->hash_tables);
         hp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
         hp.ticket = sc->hash_ticket;
         hp.lmax = N > ROSEN_LATTICE_SCAN_MAX_N ? sc->lmax : nullptr;     // short chains routed here by the env override keep the fixed shift
-        CK(cudaMemsetAsync(hp.tables, 0, threads * table_bytes, stream));      // generation 0 = empty everywhere
         CK(cudaMemsetAsync(hp.ticket, 0, sizeof(unsigned long long), stream));
         rc = rosen::launch_lattice_hash(hp, (int)threads, stream, &g_kernel);
         if (rc < 0) return fail_cuda(cudaGetLastError(), "lattice hash kernel launch");
@@ -309,15 +330,18 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
         if (warps > by_mem) warps = by_mem;
         {
             std::lock_guard<std::mutex> lock(g_mutex);
+            const size_t had = sc->hash_tables_bytes;
             if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, warps * lp.warp_bytes))) return rc;
             if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
             if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
+            const uint64_t layout = (2ull << 62) | ((uint64_t)(lp.warp_bytes >> 8) << 24) | (uint64_t)warps;
+            if ((rc = prepare_workspace(sc, layout, warps * lp.warp_bytes, sc->hash_tables_bytes != had, stream))) return rc;
         }
+        lp.gen_store = sc->hash_gen;
         lp.work = static_cast<unsigned char*>(sc->hash_tables);
         lp.rec = static_cast<rosen::ChainRecord*>(sc->hash_rec);
         lp.ticket = sc->hash_ticket;
         lp.lmax = N > ROSEN_REALSPACE_SCAN_MAX_N ? sc->lmax : nullptr;   // as in the lattice call
-        CK(cudaMemsetAsync(lp.work, 0, warps * lp.warp_bytes, stream));         // generation 0 = empty everywhere
         CK(cudaMemsetAsync(lp.ticket, 0, sizeof(unsigned long long), stream));
         rc = rosen::launch_realspace_long(lp, (int)warps, stream, &g_kernel);
         if (rc < 0) return fail_cuda(cudaGetLastError(), "real-space long-chain kernel launch");
@@ -673,6 +697,8 @@ int rosen_workspace_release(void)
     Scratch& s = g_scratch[dev];
     if (s.hash_tables || s.hash_rec || s.hash_ticket) cudaDeviceSynchronize();
     if (s.hash_tables) { cudaFree(s.hash_tables); s.hash_tables = nullptr; s.hash_tables_bytes = 0; }
+    if (s.hash_gen) { cudaFree(s.hash_gen); s.hash_gen = nullptr; }
+    s.ws_layout = 0;
     if (s.hash_rec) { cudaFree(s.hash_rec); s.hash_rec = nullptr; s.hash_rec_bytes = 0; }
     if (s.hash_ticket) { cudaFree(s.hash_ticket); s.hash_ticket = nullptr; }
     if (s.perm_thr) { cudaFree(s.perm_thr); s.perm_thr = nullptr; }

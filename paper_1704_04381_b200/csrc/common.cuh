@@ -78,6 +78,7 @@ struct HashParams {
     uint32_t   entries;         // entries per chain table (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: lanes draw chain indices from it (load balance only)
     double*    lmax;            // [kMaxPartials + 1] scratch, or null: N <= 512, fixed shift ln_shift (reading A18)
+    uint32_t*  gen_store;       // [launched threads] each thread's generation counter, kept across calls of one table layout
 };
 
 // Lattice model path (lattice_model.cu): z = 6 / 26 trial set, contact energy, records + dynamic shift.
@@ -139,6 +140,7 @@ struct RealLongParams {
     uint32_t   entries;         // cell-table entries per chain (even, >= N + 1)
     unsigned long long* ticket; // zeroed before the launch: warps draw chain indices from it (load balance only)
     double*    lmax;            // [kMaxPartials + 1] scratch, or null: N <= 2048, fixed shift ln_shift (reading A18)
+    uint32_t*  gen_store;       // [launched warps] each warp's generation counter, kept across calls of one workspace layout
 };
 
 // The ensemble reduction is tied to VIRTUAL blocks, not to the launch grid: virtual block v owns the

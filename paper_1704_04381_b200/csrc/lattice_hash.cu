@@ -9,7 +9,8 @@
 // cube to the 64-bit occupancy bitmap of its sites. An entry is 16 bytes:
 //   .x  bits 0..38   cube key (cx+2^12) | (cy+2^12) << 13 | (cz+2^12) << 26, c = coordinate >> 2 (floor)
 //       bits 39..63  the thread's chain generation (1, 2, ...): an entry whose generation differs from the current
-//                    chain's is EMPTY, so tables are never cleared between chains (one memset per launch)
+//                    chain's is EMPTY, so tables are never cleared between chains, nor between calls of the same
+//                    table layout: the counter is kept in the workspace (one memset per allocation or layout change)
 //   .y  bit (x&3) | (y&3) << 2 | (z&3) << 4 set = site occupied
 // Tables are open-addressed (Fibonacci hash of the cube key reduced by a multiply-high, linear probing, no deletions)
 // with N+1 entries (rounded up to even): a chain of N monomers touches at most N cubes, so a probe always ends at an
@@ -72,7 +73,8 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
     const int N = p.N;
     const uint32_t entries = p.entries;
     ulonglong2* table = reinterpret_cast<ulonglong2*>(p.tables) + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * entries;
-    uint32_t gen = 0;
+    const uint64_t gthread = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t gen = p.gen_store[gthread];    // generations continue across calls: entries of earlier calls stay "empty" without a memset
     uint32_t t = 0;                         // warp iteration counter (uniform): Philox blocks are drawn when t & 3 == 0
 
     // per-lane state of the chain being grown; s == 0: the lane needs a new chain
@@ -93,7 +95,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
         if (s == 0) {
             // ---- draw the next chain (timing dependent; results are not: a record is a function of the chain id)
             idx = atomicAdd(p.ticket, 1ull);
-            if (idx >= p.n_chains) break;
+            if (idx >= p.n_chains) { p.gen_store[gthread] = gen; break; }
             const uint64_t chain = p.chain_offset + idx;
             c_lo = (uint32_t)chain; c_hi = (uint32_t)(chain >> 32);
             if (++gen > kGenMax) {     // generation counter wrapped: clear the table once and start over

@@ -11,7 +11,7 @@
 //                                .x = (cx+2^14) | (cy+2^14) << 15 | (cz+2^14) << 30 | generation << 45, .y = monomer index
 // cell = floor(coordinate * inv_cell) with cell edge = candidate radius x (1 + 2^-6): the slack covers the fp32
 // rounding of the product (|x| <= 16383 b: error < 2^-9 cells), so |x_j - x_h| < radius implies cells differ by <= 1.
-// Entries of another generation are empty (one memset per launch); entries >= N + 1 > cells a chain can touch.
+// Entries of another generation are empty (the counter is kept across calls: one memset per allocation or layout change); entries >= N + 1 > cells a chain can touch.
 // Lanes 0..26 look up the 27 cells together and walk their lists in lock step; monomers that pass the candidate test
 // of realspace.cu are compacted into a shared-memory buffer, which is flushed through the trial tests whenever it
 // fills (overlap is an OR over candidates, so batching and order do not matter).
@@ -86,14 +86,15 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
     ulonglong2* table = reinterpret_cast<ulonglong2*>(base + (size_t)p.n_pad * 16);
     // this lane's cell offset among the 27 (lanes 27..31 idle in the look-up)
     const int ox = lane % 3 - 1, oy = (lane / 3) % 3 - 1, oz = lane / 9 - 1;
-    uint32_t gen = 0;
+    const uint64_t gwarp = (uint64_t)blockIdx.x * kWarpsPerBlock + warp;
+    uint32_t gen = p.gen_store[gwarp];      // generations continue across calls of one workspace layout (no memset per call)
 
     for (;;) {
         // ---- the warp draws its next chain (timing dependent; the record is a function of the chain id only)
         unsigned long long idx = 0;
         if (lane == 0) idx = atomicAdd(p.ticket, 1ull);
         idx = __shfl_sync(0xffffffffu, idx, 0);
-        if (idx >= p.n_chains) break;
+        if (idx >= p.n_chains) { if (lane == 0) p.gen_store[gwarp] = gen; break; }
         const uint64_t chain = p.chain_offset + idx;
         const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
         if (++gen > kGenMax) {

@@ -274,3 +274,24 @@ def test_config4_sweep_reduced(R):
     mx, my = sum(xs) / len(xs), sum(ys) / len(ys)
     nu = 0.5 * sum((x - mx) * (y - my) for x, y in zip(xs, ys)) / sum((x - mx) ** 2 for x in xs)
     assert 0.57 < nu < 0.63, nu
+
+
+def test_long_chain_workspace_reuse_without_clearing(R):
+    """The long-chain tables are cleared only on allocation or layout change (generation counters persist across calls):
+    repeated calls of one layout, with other layouts and the real-space long kernel in between, reproduce the same chains."""
+    ref = None
+    for rep in range(4):
+        s, t = R.rosen_lattice_generate(700, 3000, 23, outputs=("digest", "lnW"))
+        assert R.rosen_last_kernel_name().startswith("lattice_hash_kernel")
+        cur = (t["digest"].cpu().numpy().copy(), s["sum_w"], s["n_dead"])
+        if ref is None:
+            o = oracle.lattice_generate(700, 300, 23, outputs=("digest",))
+            assert np.array_equal(cur[0][:300].view(np.uint64), o.digest)
+            ref = cur
+        assert np.array_equal(cur[0], ref[0]) and cur[1] == ref[1] and cur[2] == ref[2]
+        if rep == 1:
+            R.rosen_lattice_generate(1500, 500, 1)                     # another layout in between
+        if rep == 2:
+            s2, t2 = R.rosen_realspace_generate(450, 64, 16, 1.0, 0.8, 5, outputs=("digest",))
+            o2 = oracle.realspace_generate(450, 64, 16, 1.0, 0.8, 5, outputs=("digest",))
+            assert np.array_equal(t2["digest"].cpu().numpy().view(np.uint64), o2.digest)
