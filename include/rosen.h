@@ -177,7 +177,9 @@ ROSEN_API int rosen_lattice_perm(int32_t N, uint64_t n_tours, uint64_t seed, uin
  * Enqueue-only variants: same computation, but nothing is synchronised. All outputs must be device
  * memory (outputs->memory == ROSEN_MEM_DEVICE, else ROSEN_EINVAL); `summary_device` is a DEVICE
  * pointer (may be NULL) that the second reduction pass fills on `cuda_stream`, derived fields
- * included. Used to time the path with inputs/outputs resident in HBM and to overlap calls.
+ * included. Used to time the path with inputs/outputs resident in HBM and to overlap calls. The one exception to
+ * "enqueue only": a long-chain call (N >= ROSEN_LATTICE_HASH_MIN_N / ROSEN_REALSPACE_CELL_MIN_N) that finds the library's
+ * workspace missing or too small allocates it, which synchronises the device once; repeated calls of a size do not.
  */
 ROSEN_API int rosen_lattice_generate_async(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
                                  const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
