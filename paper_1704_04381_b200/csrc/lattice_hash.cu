@@ -48,10 +48,23 @@ __device__ __forceinline__ uint64_t digest_fold(uint64_t h, uint32_t m, uint32_t
     return (h ^ (uint64_t)(m | (choice << 8))) * 0x100000001B3ull;
 }
 
-// home entry of a cube: top 32 bits of the Fibonacci hash, range-reduced to [0, entries) by a multiply-high
-__device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t entries)
+// home entry of a cube. The 2 x 2 x 2 block of cubes it belongs to (cube coordinates >> 1) is hashed to a group of 8
+// consecutive entries = one 128-byte line (Fibonacci hash, range-reduced by a multiply-high), and the low coordinate bits
+// pick the entry inside the line: a walk's consecutive cubes are neighbours in space, so they share lines instead of
+// touching one random 32-byte sector each (DRAM bytes per step: section 12). Probing stays linear over the whole table.
+__device__ __forceinline__ uint32_t slot_of_local(uint64_t cube, uint32_t entries)
 {
-    return __umulhi((uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> 32), entries);
+    constexpr uint64_t kLow = 1ull | (1ull << kCubeField) | (1ull << (2 * kCubeField));
+    const uint32_t low = (uint32_t)(cube & 1ull) | ((uint32_t)(cube >> (kCubeField - 1)) & 2u) | ((uint32_t)(cube >> (2 * kCubeField - 2)) & 4u);
+    return __umulhi((uint32_t)(((cube & ~kLow) * 0x9E3779B97F4A7C15ull) >> 32), entries >> 3) * 8u + low;
+}
+
+// Very long chains fill whole lines with neighbouring cubes and then probe through them (N = 10000: 104 -> 124 ms with the
+// line-local hash), so from kLocalHashMaxN on every cube is hashed on its own.
+constexpr int kLocalHashMaxN = 4096;
+__device__ __forceinline__ uint32_t slot_of(uint64_t cube, uint32_t entries, bool local)
+{
+    return local ? slot_of_local(cube, entries) : __umulhi((uint32_t)((cube * 0x9E3779B97F4A7C15ull) >> 32), entries);
 }
 
 // three-way select by axis
@@ -72,6 +85,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
 
     const int N = p.N;
     const uint32_t entries = p.entries;
+    const bool local_hash = N <= kLocalHashMaxN;
     ulonglong2* table = reinterpret_cast<ulonglong2*>(p.tables) + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * entries;
     const uint64_t gthread = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t gen = p.gen_store[gthread];    // generations continue across calls: entries of earlier calls stay "empty" without a memset
@@ -105,7 +119,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             tag = (uint64_t)gen << kGenShift;
             // ---- L0: r_0 = origin; every entry is empty for a new generation, so the origin's cube takes its home slot
             cube = kOriginCube; bits = 1ull; l = 0u;
-            slot = slot_of(cube, entries);
+            slot = slot_of(cube, entries, local_hash);
             table[slot] = make_ulonglong2(cube | tag, bits);
             x = y = z = sx = sy = sz = 0; s2 = 0; lnW = 0.0; s = 1;
             dg = 0xCBF29CE484222325ull;
@@ -139,7 +153,7 @@ __global__ void __launch_bounds__(256, 3) lattice_hash_kernel(const HashParams p
             nl[a] = (up ? l - (3u << (2 * a)) : l + (3u << (2 * a))) & 63u;
             // no face on this axis: probe the growth point's own entry instead (cached, never a match for nkey, never
             // empty) so that the load needs no branch; its result is not used
-            nslot[a] = need[a] ? slot_of(nkey[a], entries) : slot;
+            nslot[a] = need[a] ? slot_of(nkey[a], entries, local_hash) : slot;
             first[a] = table[nslot[a]];
         }
         uint32_t pend = 0;
@@ -302,7 +316,7 @@ __global__ void __launch_bounds__(256) reduce_records_kernel(const ChainRecord* 
 
 uint32_t hash_entries(int32_t N)
 {
-    return ((uint32_t)N + 2u) & ~1u;                   // even and >= N + 1 > cubes one chain can touch
+    return ((uint32_t)N + 8u) & ~7u;                   // a multiple of 8 (whole 128-byte lines) and >= N + 1 > cubes one chain can touch
 }
 
 int hash_max_threads(int* threads_out)
