@@ -55,7 +55,7 @@ LONG_REALSPACE = (Workload("realspace_long_N4096_k16_2p16", "realspace", 4096, 1
 MODELS = (Workload("lattice_z26_N64_2p20", "lattice", 64, 1 << 20, 19, z=26, beta_eps=0.0),
           Workload("lattice_z6_contact0.3_N64_2p20", "lattice", 64, 1 << 20, 19, z=6, beta_eps=0.3),
           Workload("realspace_well1.5_0.4_N64_k16_2p20", "realspace", 64, 1 << 20, 19, 16, 1.0, 1.0, beta_eps=0.4, lam=1.5),
-          Workload("lattice_perm_N256_2p16", "lattice", 256, 1 << 16, 19, perm=(0.5, 2.0)))
+          Workload("lattice_perm_N256_2p20", "lattice", 256, 1 << 20, 19, perm=(0.5, 2.0)))
 
 CONFIGS = {w.name: w for w in (CONFIG_1, CONFIG_2, CONFIG_3, *CONFIG_4, CONFIG_5, *LONG_LATTICE, *LONG_REALSPACE, *MODELS)}
 
