@@ -38,6 +38,8 @@ struct Scratch {
     void*          hash_tables = nullptr;  size_t hash_tables_bytes = 0;
     void*          hash_rec = nullptr;     size_t hash_rec_bytes = 0;
     unsigned long long* hash_ticket = nullptr;
+    uint32_t*      done_flags = nullptr;   // [kMaxPartials] mapped pinned host memory: virtual blocks whose outputs are stored
+    cudaStream_t   copy_stream = nullptr;  // device->host copies of finished conformations while the kernel runs
     uint32_t*      hash_gen = nullptr;     // [kMaxGenSlots] generation counters of the long-chain kernels' threads / warps
     uint64_t       ws_layout = 0;          // signature of the table layout the workspace was last cleared for (0: none)
     double*        perm_thr = nullptr;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
@@ -68,6 +70,14 @@ int get_scratch(Scratch** out)
             return fail_cuda(e, "per-device scratch allocation");
         }
         s.summary_dev = sd; s.vb_counter = vc; s.lmax = lm; s.summary_host = sh; s.dev = d;
+        // host-pointer calls stage through stream-ordered allocations: keep freed staging memory in the pool instead of
+        // returning gigabytes to the driver at every synchronisation (config 5: 3.2 GB per call)
+        cudaMemPool_t pool = nullptr;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
+            uint64_t keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
     }
     *out = &s;
     return ROSEN_OK;
@@ -94,6 +104,35 @@ int prepare_workspace(Scratch* sc, uint64_t layout, size_t table_bytes_total, bo
         CK(cudaMemsetAsync(sc->hash_gen, 0, kMaxGenSlots * sizeof(uint32_t), stream));
         sc->ws_layout = layout;
     }
+    return ROSEN_OK;
+}
+
+// Host conformation buffers (ROSEN_MEM_HOST + conf): the generation kernel raises a flag in mapped host memory for every
+// virtual block whose outputs are stored; this loop copies the finished chain ranges device -> host on a second stream while
+// the kernel is still running, so the PCIe transfer of the dump (3.2 GB at config 5) overlaps the generation instead of following it.
+int stream_conf_out(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, void* conf_host, size_t row_bytes,
+                    uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks)
+{
+    volatile uint32_t* flags = sc->done_flags;
+    const uint32_t batch = n_vblocks / 32 > 8 ? n_vblocks / 32 : 8;       // virtual blocks per copy: large transfers, ~32 per call
+    uint32_t next = 0, seen = 0;
+    bool kernel_over = false;
+    while (next < n_vblocks) {
+        while (seen < n_vblocks && flags[seen] != 0u) ++seen;
+        if (seen - next >= batch || (seen == n_vblocks && seen > next) || (kernel_over && seen > next)) {
+            const uint64_t c0 = (uint64_t)next * chunk, c1 = (uint64_t)seen * chunk < n_chains ? (uint64_t)seen * chunk : n_chains;
+            CK(cudaMemcpyAsync(static_cast<char*>(conf_host) + c0 * row_bytes, static_cast<const char*>(conf_dev) + c0 * row_bytes,
+                               (c1 - c0) * row_bytes, cudaMemcpyDeviceToHost, sc->copy_stream));
+            next = seen;
+            continue;
+        }
+        if (kernel_over) break;                                           // flags missing although the kernel ended: launch failed
+        const cudaError_t q = cudaStreamQuery(gen_stream);
+        if (q == cudaSuccess) { kernel_over = true; continue; }           // one more pass over the flags
+        if (q != cudaErrorNotReady) return fail_cuda(q, "generation kernel");
+    }
+    CK(cudaStreamSynchronize(sc->copy_stream));
+    if (next < n_vblocks) { std::snprintf(g_err, sizeof(g_err), "generation kernel ended without storing every virtual block"); return ROSEN_ECUDA; }
     return ROSEN_OK;
 }
 
@@ -170,14 +209,14 @@ int stage_outputs(const rosen_outputs* o, const Sizes& z, cudaStream_t stream, S
     return ROSEN_OK;
 }
 
-int copy_back(const rosen_outputs* o, const Sizes& z, const Staging& st, cudaStream_t stream)
+int copy_back(const rosen_outputs* o, const Sizes& z, const Staging& st, cudaStream_t stream, bool conf_done = false)
 {
     if (!o || !st.staged) return ROSEN_OK;
     if (o->lnW) CK(cudaMemcpyAsync(o->lnW, st.dev.lnW, z.lnW, cudaMemcpyDeviceToHost, stream));
     if (o->alive) CK(cudaMemcpyAsync(o->alive, st.dev.alive, z.alive, cudaMemcpyDeviceToHost, stream));
     if (o->m_seq) CK(cudaMemcpyAsync(o->m_seq, st.dev.m_seq, z.m_seq, cudaMemcpyDeviceToHost, stream));
     if (o->digest) CK(cudaMemcpyAsync(o->digest, st.dev.digest, z.digest, cudaMemcpyDeviceToHost, stream));
-    if (o->conf) CK(cudaMemcpyAsync(o->conf, st.dev.conf, z.conf, cudaMemcpyDeviceToHost, stream));
+    if (o->conf && !conf_done) CK(cudaMemcpyAsync(o->conf, st.dev.conf, z.conf, cudaMemcpyDeviceToHost, stream));
     if (o->ree2) CK(cudaMemcpyAsync(o->ree2, st.dev.ree2, z.ree2, cudaMemcpyDeviceToHost, stream));
     if (o->rg2) CK(cudaMemcpyAsync(o->rg2, st.dev.rg2, z.rg2, cudaMemcpyDeviceToHost, stream));
     return ROSEN_OK;
@@ -194,7 +233,7 @@ void derive(rosen_summary* s)
 // After the generation kernel: second reduction pass, summary copy, host staging copies, sync.
 // summary (host) and summary_dev (device) are both optional; the finalize kernel runs if either is set.
 int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const double* ln_shift_dev, const rosen_outputs* outputs, const Sizes& z,
-           Staging& st, rosen_summary* summary, rosen_summary* summary_dev, cudaStream_t stream)
+           Staging& st, rosen_summary* summary, rosen_summary* summary_dev, cudaStream_t stream, bool conf_done = false)
 {
     if (summary || summary_dev) {
         rosen_summary* target = summary_dev ? summary_dev : sc->summary_dev;
@@ -203,7 +242,7 @@ int finish(Scratch* sc, int grid, uint64_t n_chains, double ln_shift, const doub
         ++g_launches;
         if (summary) CK(cudaMemcpyAsync(sc->summary_host, target, sizeof(rosen_summary), cudaMemcpyDeviceToHost, stream));
     }
-    int rc = copy_back(outputs, z, st, stream);
+    int rc = copy_back(outputs, z, st, stream, conf_done);
     if (rc) return rc;
     st.release();
     if (summary || (outputs && outputs->memory == ROSEN_MEM_HOST)) CK(cudaStreamSynchronize(stream));
@@ -357,11 +396,27 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
     p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
     rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks, 256u);
     CK(cudaMemsetAsync(sc->vb_counter, 0, sizeof(uint32_t), stream));
+    // large dump into host memory: stream the finished conformations out while the kernel runs
+    const bool overlap = st.staged && outputs->conf != nullptr && p.n_vblocks >= 64;
+    if (overlap) {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if (!sc->done_flags) CK(cudaHostAlloc(reinterpret_cast<void**>(&sc->done_flags), rosen::kMaxPartials * sizeof(uint32_t), cudaHostAllocMapped));
+        if (!sc->copy_stream) CK(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
+    }
+    if (overlap) {
+        CK(cudaStreamSynchronize(stream));                               // staging buffers exist before the copy stream reads them
+        std::memset(sc->done_flags, 0, p.n_vblocks * sizeof(uint32_t));
+        uint32_t* dflags = nullptr;
+        CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dflags), sc->done_flags, 0));
+        p.done = dflags;
+    }
     int grid = 0;
     rc = rosen::launch_realspace(p, stream, &g_kernel, &grid);
     if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "real-space kernel launch");
     g_launches += rc;
-    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, outputs, z, st, summary, summary_dev, stream);
+    if (overlap && (rc = stream_conf_out(sc, stream, st.dev.conf, outputs->conf, (size_t)N * 3 * sizeof(float), n_chains, p.chunk, p.n_vblocks)))
+        return rc;
+    return finish(sc, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, outputs, z, st, summary, summary_dev, stream, overlap);
 }
 
 // Fixed-point Boltzmann factors of the model calls: Q[c] = round(p_c 2^16), p_0 = 1, p_c = p_{c-1} q in fp64.

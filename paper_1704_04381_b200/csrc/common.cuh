@@ -50,6 +50,8 @@ struct RealParams {
     uint32_t   chunk;           // chains per virtual block (multiple of 256)
     uint32_t   n_vblocks;
     uint32_t*  vb_counter;      // as in LatticeParams
+    uint32_t*  done;            // null, or [n_vblocks] flags in mapped host memory: set when a virtual block's outputs are stored
+                                // (the host streams finished conformations out while the kernel runs: DESIGN.md 5.4)
     // square-well model (rosen_realspace_generate_model): rec != nullptr selects the WELL kernels
     float        well2;         // fl32(fl32(lambda sigma)^2)
     ChainRecord* rec;           // [n_chains]: per-chain records instead of block partials (shift = largest lnW of the call)

@@ -397,6 +397,11 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
 
     if (WELL) __syncthreads();      // the sums are formed from the records afterwards; the ticket still needs the barrier
     else block_reduce_store(acc, scratch, p.partials + vb);
+    if (p.done != nullptr) {        // every thread's stores of this virtual block are visible system-wide before the flag is
+        __threadfence_system();
+        __syncthreads();
+        if (threadIdx.x == 0) { *reinterpret_cast<volatile uint32_t*>(p.done + vb) = 1u; __threadfence_system(); }
+    }
     }
 }
 

@@ -232,3 +232,18 @@ def test_direction_map_exhaustive_z(R):
         assert np.array_equal(got[:, 2], z64.astype(np.float32))
         assert np.array_equal(got[:, 0].view(np.uint32), ux.view(np.uint32))
         assert np.array_equal(got[:, 1].view(np.uint32), uy.view(np.uint32))
+
+
+def test_host_conf_streamed_out_while_the_kernel_runs(R):
+    """ROSEN_MEM_HOST + conf with >= 64 virtual blocks: finished chain ranges are copied device -> host on a second stream
+    while the kernel still runs. Same bits as the device-buffer call, ragged last virtual block included."""
+    N, n, k = 24, 70001, 16
+    s_d, t_d = R.rosen_realspace_generate(N, n, k, 1.0, 0.9, 31, outputs=("conf", "lnW", "digest"))
+    for _ in range(2):
+        s_h, t_h = R.rosen_realspace_generate(N, n, k, 1.0, 0.9, 31, outputs=("conf", "lnW", "digest"), host_outputs=True)
+        assert s_h == s_d
+        for key in ("conf", "lnW", "digest"):
+            assert not t_h[key].is_cuda
+            assert np.array_equal(t_h[key].numpy(), t_d[key].cpu().numpy()), key
+    o = oracle.realspace_generate(N, 64, k, 1.0, 0.9, 31, chain_offset=n - 64, outputs=("conf",))
+    assert np.array_equal(t_h["conf"].numpy()[n - 64:], o.conf)
