@@ -285,7 +285,10 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
         {
             std::lock_guard<std::mutex> lock(g_mutex);
             const size_t had = sc->hash_tables_bytes;
-            if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, threads * table_bytes))) return rc;
+            // a smaller or busy GPU: fewer resident tables (results do not depend on how many threads share the chains)
+            while ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, threads * table_bytes)) == ROSEN_ENOMEM && threads > 256)
+                threads = (threads / 2 + 255) / 256 * 256;
+            if (rc) return rc;
             if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
             if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
             if (threads > kMaxGenSlots) threads = kMaxGenSlots;
@@ -370,7 +373,9 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
         {
             std::lock_guard<std::mutex> lock(g_mutex);
             const size_t had = sc->hash_tables_bytes;
-            if ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, warps * lp.warp_bytes))) return rc;
+            while ((rc = grow(&sc->hash_tables, &sc->hash_tables_bytes, warps * lp.warp_bytes)) == ROSEN_ENOMEM && warps > 8)
+                warps = (warps / 2 + 7) / 8 * 8;
+            if (rc) return rc;
             if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
             if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
             const uint64_t layout = (2ull << 62) | ((uint64_t)(lp.warp_bytes >> 8) << 24) | (uint64_t)warps;
