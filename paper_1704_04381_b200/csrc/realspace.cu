@@ -245,9 +245,7 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
             // ---- R2: monomers j <= s-2 (slots 0..s-2; r_{s-1} itself is stored at the end of this step), 32 per pass:
             // mark those within the conservative radius of r_{s-1}, then test the trials against the marked ones
             // (overlap is an OR over monomers: order and batching are irrelevant)
-            for (int j0 = 0; j0 < s - 1; j0 += 32) {
-                const float4* pb = R4 + j0;
-                uint32_t mask = candidate_bits<G>(pb, s - 1 - j0, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
+            auto test_marked = [&](uint32_t mask, const float4* pb) {
                 while (mask) {
                     const uint32_t bpos = bfind(mask);
                     mask ^= 1u << bpos;
@@ -260,6 +258,22 @@ __global__ void __launch_bounds__(256, 3) realspace_kernel(const RealParams p)
                         if (WELL) nwell[i] += d2 < p.well2 ? 1u : 0u;
                     }
                 }
+            };
+            {
+                const int cnt = s - 1;
+                int j0 = 0;
+                if constexpr (G == 32) {
+                    // two passes per iteration while two remain: independent loads and distance chains, half the loop overhead
+                    for (; j0 + 32 < cnt; j0 += 64) {
+                        const float4* pb = R4 + j0;
+                        const uint32_t m0 = candidate_bits<G>(pb, 32, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
+                        const uint32_t m1 = candidate_bits<G>(pb + 32, 32, gl, gshift, gmask, hx, hy, hz, p.prefilter2);
+                        test_marked(m0, pb);
+                        test_marked(m1, pb + 32);
+                    }
+                }
+                for (; j0 < cnt; j0 += 32)
+                    test_marked(candidate_bits<G>(R4 + j0, cnt - j0, gl, gshift, gmask, hx, hy, hz, p.prefilter2), R4 + j0);
             }
 
             // ---- m_s and the number of free trials of lower lanes (trial order = lane order, then i)
