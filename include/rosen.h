@@ -19,8 +19,10 @@
  *   - Chain ids: chain i of a call has id chain_offset + i. Every per-chain result is a pure
  *     function of (seed, id, parameters): any sub-range reproduces bit-identically, which is how
  *     multi-GPU sharding, resume and sampled parity checks work.
- *   - Calls on one device share that device's scratch (block partials; the long-chain workspace): enqueue the calls
- *     of a device on one stream, or order them with events; calls on different devices are independent.
+ *   - Calls on one device share that device's scratch (block partials; the long-chain workspace). The library keeps them
+ *     apart itself: host threads are serialised per device for the duration of a call, and a call enqueued on another
+ *     stream than the previous call of that device first waits (cudaStreamWaitEvent) for that call's work. Calls on
+ *     different devices are independent.
  *   - There is no CPU fallback: without a CUDA device every generate call fails with ROSEN_ECUDA.
  */
 #ifndef ROSEN_H

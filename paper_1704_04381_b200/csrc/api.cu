@@ -28,6 +28,13 @@ int fail_cuda(cudaError_t e, const char* what)
 #define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail_cuda(e_, #call); } while (0)
 
 // Per-device scratch: block partials + one total, and a pinned host mirror of the total.
+struct Scratch;
+// RAII: serialises the calls of one device (host side) and orders them across streams (device side).
+struct CallGuard {
+    Scratch* sc = nullptr; cudaStream_t stream = nullptr;
+    int enter(Scratch* s, cudaStream_t st);
+    ~CallGuard();
+};
 struct Scratch {
     Partial*       dev = nullptr;          // [kMaxPartials] block partials
     rosen_summary* summary_dev = nullptr;  // written by finalize_kernel
@@ -42,7 +49,13 @@ struct Scratch {
     cudaStream_t   copy_stream = nullptr;  // device->host copies of finished conformations while the kernel runs
     uint32_t*      hash_gen = nullptr;     // [kMaxGenSlots] generation counters of the long-chain kernels' threads / warps
     uint64_t       ws_layout = 0;          // signature of the table layout the workspace was last cleared for (0: none)
-    double*        perm_thr = nullptr;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
+    double*        perm_thr = nullptr;
+    // calls of one device share everything above: host threads take call_mutex for the whole call, and a call on another
+    // stream than the previous one first waits for that call's last enqueued work (last_done)
+    std::mutex     call_mutex;
+    cudaEvent_t    last_done = nullptr;
+    cudaStream_t   last_stream = nullptr;
+    bool           have_last = false;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
 };
 constexpr size_t kHashTableCap = (size_t)12 << 30;  // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
@@ -81,6 +94,22 @@ int get_scratch(Scratch** out)
     }
     *out = &s;
     return ROSEN_OK;
+}
+
+int CallGuard::enter(Scratch* s, cudaStream_t st)
+{
+    s->call_mutex.lock();
+    sc = s; stream = st;
+    if (!s->last_done) CK(cudaEventCreateWithFlags(&s->last_done, cudaEventDisableTiming));
+    if (s->have_last && s->last_stream != st) CK(cudaStreamWaitEvent(st, s->last_done, 0));
+    return ROSEN_OK;
+}
+CallGuard::~CallGuard()
+{
+    if (!sc) return;
+    if (sc->last_done && cudaEventRecord(sc->last_done, stream) == cudaSuccess) { sc->last_stream = stream; sc->have_last = true; }
+    else cudaGetLastError();
+    sc->call_mutex.unlock();
 }
 
 int grow(void** ptr, size_t* have, size_t need)
@@ -260,6 +289,8 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
     Scratch* sc = nullptr;
     int rc = get_scratch(&sc);
     if (rc) return rc;
+    CallGuard guard;
+    if ((rc = guard.enter(sc, stream))) return rc;
     const Sizes z = output_sizes(N, n_chains, sizeof(int32_t));
     Staging st;
     if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
@@ -336,6 +367,8 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
     Scratch* sc = nullptr;
     int rc = get_scratch(&sc);
     if (rc) return rc;
+    CallGuard guard;
+    if ((rc = guard.enter(sc, stream))) return rc;
     const Sizes z = output_sizes(N, n_chains, sizeof(float));
     Staging st;
     if ((rc = stage_outputs(outputs, z, stream, &st))) return rc;
@@ -445,6 +478,8 @@ int lattice_model_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t cha
     Scratch* sc = nullptr;
     int rc = get_scratch(&sc);
     if (rc) return rc;
+    CallGuard guard;
+    if ((rc = guard.enter(sc, stream))) return rc;
     const Sizes zs = output_sizes(N, n_chains, sizeof(int32_t));
     Staging st;
     if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;
@@ -482,6 +517,8 @@ int realspace_model_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float b
     Scratch* sc = nullptr;
     int rc = get_scratch(&sc);
     if (rc) return rc;
+    CallGuard guard;
+    if ((rc = guard.enter(sc, stream))) return rc;
     const Sizes zs = output_sizes(N, n_chains, sizeof(float));
     Staging st;
     if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;
@@ -530,6 +567,8 @@ int perm_impl(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset, 
     Scratch* sc = nullptr;
     int rc = get_scratch(&sc);
     if (rc) return rc;
+    CallGuard guard;
+    if ((rc = guard.enter(sc, stream))) return rc;
     const Sizes zs = output_sizes(N, n_tours, sizeof(int32_t));
     Staging st;
     if ((rc = stage_outputs(outputs, zs, stream, &st))) return rc;

@@ -295,3 +295,25 @@ def test_long_chain_workspace_reuse_without_clearing(R):
             s2, t2 = R.rosen_realspace_generate(450, 64, 16, 1.0, 0.8, 5, outputs=("digest",))
             o2 = oracle.realspace_generate(450, 64, 16, 1.0, 0.8, 5, outputs=("digest",))
             assert np.array_equal(t2["digest"].cpu().numpy().view(np.uint64), o2.digest)
+
+
+def test_concurrent_calls_from_threads_and_streams(R):
+    """Calls of one device share scratch (block partials, records, tables): the library serialises host threads and orders
+    the streams itself, so concurrent callers get the results of sequential calls."""
+    import threading
+    import torch
+    jobs = [(48, 30000, 100 + i) for i in range(4)] + [(300, 2000, 200 + i) for i in range(2)]
+    want = [R.rosen_lattice_generate(N, n, seed, outputs=("digest",)) for N, n, seed in jobs]
+    got = [None] * len(jobs)
+
+    def run(i):
+        N, n, seed = jobs[i]
+        st = torch.cuda.Stream()
+        for _ in range(3):
+            got[i] = R.rosen_lattice_generate(N, n, seed, outputs=("digest",), stream=st)
+
+    th = [threading.Thread(target=run, args=(i,)) for i in range(len(jobs))]
+    for t in th: t.start()
+    for t in th: t.join()
+    for (s0, t0), (s1, t1) in zip(want, got):
+        assert s0 == s1 and torch.equal(t0["digest"], t1["digest"])
