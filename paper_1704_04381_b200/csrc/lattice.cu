@@ -44,9 +44,9 @@ __host__ __device__ inline int stride_of(int N) { return 2 * half4_of(N) + 4; }
 // (keys 1, 3) -- 5.25 issue slots against 8 for the compare scan.
 // -----------------------------------------------------------------------------------------------------
 struct DpTables {
-    uint2    lut[64];   // index = (b0,b1,b8,b9,b16,b17) of the XOR. .x: bits 0-2 = m, bits 4+4i..6+4i = i-th free
-                        // direction; .y: histogram increment 1 << 8*(m-2) for m = 2..5
-    int32_t  delta[8];  // key delta per direction
+    uint4    lut[64];   // index = (b0,b1,b8,b9,b16,b17) of the XOR. Bytes 0..5 of (.x, .y) = 4 * (i-th free direction), picked
+                        // with one byte permute; .z: histogram increment 1 << 8*(m-2) for m = 2..5; .w = m
+    int32_t  delta[8];  // key delta per direction; [6], [7]: unused directions, hold the byte selectors 0x100, 0x10000
     double   ln_m[8];
 };
 
@@ -57,14 +57,15 @@ __device__ __forceinline__ void build_dp_tables(DpTables* t)
         const int b0 = idx & 1, b1 = (idx >> 1) & 1, b8 = (idx >> 2) & 1, b9 = (idx >> 3) & 1, b16 = (idx >> 4) & 1, b17 = (idx >> 5) & 1;
         // XOR patterns: +x 0x1, -x 0xFFFFFFFF, +y 0x100, -y 0xFFFFFF00, +z 0x10000, -z 0xFFFF0000
         const int occ_d[6] = { b0 ^ b1, b1, b8 ^ b9, b9 ^ b1, b16 ^ b17, b17 ^ b9 };
-        uint32_t e = 0, m = 0;
+        uint64_t e = 0;
+        uint32_t m = 0;
         for (int d = 0; d < 6; ++d)
-            if (!occ_d[d]) { e |= (uint32_t)d << (4 + 4 * m); ++m; }
-        t->lut[idx] = make_uint2(e | m, (m >= 2 && m <= 5) ? 1u << (8 * (m - 2)) : 0u);
+            if (!occ_d[d]) { e |= (uint64_t)(4 * d) << (8 * m); ++m; }
+        t->lut[idx] = make_uint4((uint32_t)e, (uint32_t)(e >> 32), (m >= 2 && m <= 5) ? 1u << (8 * (m - 2)) : 0u, m);
     }
     if (threadIdx.x < 8) {
         const int d = threadIdx.x;
-        t->delta[d] = d < 6 ? ((d & 1) ? -1 : 1) * (1 << (B * (d >> 1))) : 0;
+        t->delta[d] = d < 6 ? ((d & 1) ? -1 : 1) * (1 << (B * (d >> 1))) : (d == 6 ? 0x100 : 0x10000);
         t->ln_m[d] = d == 0 ? -CUDART_INF : log((double)d);
     }
 }
@@ -162,19 +163,19 @@ __device__ __forceinline__ uint32_t scan_dpw(uint32_t addr, uint32_t T, uint32_t
     return A;
 }
 
-__device__ __forceinline__ uint2 lds64(uint32_t a) { uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ uint4 lds128(uint32_t a) { uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts128(uint32_t a, uint32_t v) { asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" :: "r"(a), "r"(v), "r"(0u) : "memory"); }
 
-// MODE 0: N <= 64, 8-bit fields, lnW from an m histogram. MODE 1: 64 < N <= 128, 8-bit fields, lnW as a running fp64 sum in
+// MODE 0: N <= 64, 8-bit fields, lnW from an m histogram; MODE 3: the same for N = 0 (mod 4), without the per-step s < N test. MODE 1: 64 < N <= 128, 8-bit fields, lnW as a running fp64 sum in
 // step order (lnW crosses 128 there, where the oracle's step-by-step sum rounds every ln 5 it adds the same way -- a systematic
 // 6e-13 relative to the histogram's more accurate value; following the oracle's order keeps the ensemble sums within 1e-13).
 // MODE 2 ("wide"): 128 < N <= 512, 10-bit fields, running sum.
 template <int MODE, bool DIGEST, bool TRAJ>
 __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
 {
-    constexpr bool WIDE = MODE == 2, RUNSUM = MODE >= 1;
+    constexpr bool WIDE = MODE == 2, RUNSUM = MODE == 1 || MODE == 2, FULL4 = MODE == 3, SHORT = MODE == 0 || MODE == 3;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     DpTables* tab = reinterpret_cast<DpTables*>(smem_raw);
     Partial* scratch = reinterpret_cast<Partial*>(smem_raw + sizeof(DpTables));
@@ -188,15 +189,21 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
     const int half4 = half4_of(N), stride = stride_of(N);
     uint32_t* ev = chains + (size_t)threadIdx.x * stride;   // monomers 0,2,4,...
     uint32_t* od = ev + half4;                              // monomers 1,3,5,...
-    const uint32_t lut_addr = (uint32_t)__cvta_generic_to_shared(tab->lut);
-    const uint32_t delta_addr = (uint32_t)__cvta_generic_to_shared(tab->delta);
+    uint32_t lut_addr = (uint32_t)__cvta_generic_to_shared(tab->lut);
+    uint32_t delta_addr = (uint32_t)__cvta_generic_to_shared(tab->delta);
     const uint32_t ev_addr = (uint32_t)__cvta_generic_to_shared(ev);
     const uint32_t od_addr = ev_addr + (uint32_t)half4 * 4u;
+    // Opaque copies: otherwise the compiler re-derives the shared-window addresses and the three byte selectors of the
+    // coordinate sums with uniform-datapath instructions in every step (7 issue slots per step in the round-1 SASS).
+    if (SHORT) asm volatile("" : "+r"(lut_addr), "+r"(delta_addr));      // (measured: helps N <= 64, costs 10 % at N = 128)
 
     build_dp_tables<B>(tab);
     __syncthreads();
 
     const uint32_t per_thread = p.chunk / blockDim.x;
+    // the byte selectors of the coordinate sums come from memory so that they live in registers (as immediates they are
+    // re-materialised by three uniform moves in every step)
+    const int sel_y = SHORT ? tab->delta[6] : 0x100, sel_z = SHORT ? tab->delta[7] : 0x10000, sel_x = sel_y >> 8;
 
     __shared__ uint32_t vb_ticket;
     for (;;) {
@@ -231,25 +238,26 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const int s = 4 * q + k;
-                    if (s == 0 || s >= N) continue;
+                    if (FULL4) { if (k == 0 && q == 0) continue; }            // N = 0 (mod 4): every block serves four steps, but s = 0
+                    else if (s == 0 || s >= N) continue;
 
                     // L2
                     uint32_t A = 0;
                     const uint32_t T = (uint32_t)(((s >> 1) + 3) >> 2);
                     if (T != 0u) A = WIDE ? scan_dpw((k & 1) ? od_addr : ev_addr, T, h) : scan_dp((k & 1) ? od_addr : ev_addr, T, h);
-                    uint32_t li;                                              // 8 * (b0,b1,bB,bB+1,b2B,b2B+1)
-                    if (WIDE) { const uint32_t x = A & 0x00300C03u; li = ((x | (x >> 8) | (x >> 16)) & 0x3Fu) << 3; }
-                    else li = (((A & 0x00030303u) * 0x00010410u) >> 13) & 0x1F8u;
-                    const uint2 le = lds64(lut_addr + li);
-                    const uint32_t m = le.x & 7u;
+                    uint32_t li;                                              // 16 * (b0,b1,bB,bB+1,b2B,b2B+1)
+                    if (WIDE) { const uint32_t x = A & 0x00300C03u; li = ((x | (x >> 8) | (x >> 16)) & 0x3Fu) << 4; }
+                    else li = (((A & 0x00030303u) * 0x00010410u) >> 12) & 0x3F0u;
+                    const uint4 le = lds128(lut_addr + li);
+                    const uint32_t m = le.w;
 
                     // L3
-                    if (RUNSUM) lnW_w += tab->ln_m[m]; else hist += le.y;
+                    if (RUNSUM) lnW_w += tab->ln_m[m]; else hist += le.z;
                     if (TRAJ && mrow) mrow[s - 1] = dead == 0u ? (uint8_t)m : (uint8_t)0;
 
                     // L4
                     const uint32_t sel = __umulhi(w[k], m);
-                    const uint32_t d4 = (le.x >> (4u * sel + 2u)) & 0x1Cu;     // 4 * direction
+                    const uint32_t d4 = __byte_perm(le.x, le.y, sel) & 0xFFu;   // 4 * direction
                     if (DIGEST) { if (dead == 0u) dg = digest_fold(dg, m, m ? (d4 >> 2) : 0xFFu); }
                     dead = (m == 0u && dead == 0u) ? (uint32_t)s : dead;
                     h += lds32(delta_addr + d4);
@@ -264,7 +272,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                     } else {
                         const int sg = (int)(h ^ kOrigin);
                         s2 = __dp4a(sg, sg, s2);
-                        sx = __dp4a(sg, 0x00000001, sx); sy = __dp4a(sg, 0x00000100, sy); sz = __dp4a(sg, 0x00010000, sz);
+                        sx = __dp4a(sg, sel_x, sx); sy = __dp4a(sg, sel_y, sy); sz = __dp4a(sg, sel_z, sz);
                     }
                 }
             }
@@ -372,7 +380,8 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
     if (p.N <= 128) {   // every scanned difference |dx|,|dy|,|dz| <= s-1-j <= 126 fits a signed byte: byte-dot-product scan
         *kernel_name = traj ? (digest ? "lattice_dp_kernel<digest,traj>" : "lattice_dp_kernel<traj>")
                             : (digest ? "lattice_dp_kernel<digest>" : "lattice_dp_kernel");
-        return p.N <= 64 ? launch_dp<0>(p, stream, grid_out) : launch_dp<1>(p, stream, grid_out);
+        if (p.N <= 64) return (p.N & 3) == 0 ? launch_dp<3>(p, stream, grid_out) : launch_dp<0>(p, stream, grid_out);
+        return launch_dp<1>(p, stream, grid_out);
     }
     // 10-bit fields (|d| <= 510 < 2^9, 128 < N <= 512): power-of-two test + byte-sum scan
     *kernel_name = traj ? (digest ? "lattice_dp_kernel<wide,digest,traj>" : "lattice_dp_kernel<wide,traj>")
