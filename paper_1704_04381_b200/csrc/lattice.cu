@@ -81,13 +81,14 @@ __device__ __forceinline__ void build_dp_tables(DpTables* t)
 
 // addr: shared byte address of the parity array, T >= 1 chunks of 4 keys, h: key of r_{s-1}. Returns the XOR.
 // Chunks are double-buffered; the load runs at most one chunk past the T-th (inside the thread's own region).
-__device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t h)
+// minus1 = 0xFFFFFFFF in a register that the caller loaded from memory (as an immediate it is re-materialised in every call)
+__device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t h, uint32_t minus1)
 {
     uint32_t A;
     asm volatile("{\n"
         ".reg .pred q, p1, p3;\n"
         ".reg .b32 a0, a1, a2, a3, b0, b1, b2, b3, ad, od, cnt, A, m1, w0, w1, w2, w3, t0, t1, t2, t3;\n"
-        "mov.u32 ad, %1; mov.u32 cnt, %2; mov.u32 A, 0; mov.u32 m1, 0xFFFFFFFF;\n"
+        "mov.u32 ad, %1; mov.u32 cnt, %2; mov.u32 A, 0; mov.u32 m1, %4;\n"
         "ld.shared.v4.b32 {a0, a1, a2, a3}, [ad];\n"
         "and.b32 od, cnt, 1;\n"
         "setp.eq.u32 q, od, 0;\n"
@@ -110,7 +111,7 @@ __device__ __forceinline__ uint32_t scan_dp(uint32_t addr, uint32_t T, uint32_t 
         "mov.u32 %0, A;\n"
         "}\n"
         : "=r"(A)
-        : "r"(addr), "r"(T), "r"(h)
+        : "r"(addr), "r"(T), "r"(h), "r"(minus1)
         : "memory");
     return A;
 }
@@ -203,6 +204,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
     const uint32_t per_thread = p.chunk / blockDim.x;
     // the byte selectors of the coordinate sums come from memory so that they live in registers (as immediates they are
     // re-materialised by three uniform moves in every step)
+    const uint32_t minus1 = SHORT ? (uint32_t)tab->delta[1] : 0xFFFFFFFFu;      // delta of -x = -1
     const int sel_y = SHORT ? tab->delta[6] : 0x100, sel_z = SHORT ? tab->delta[7] : 0x10000, sel_x = sel_y >> 8;
 
     __shared__ uint32_t vb_ticket;
@@ -244,7 +246,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
                     // L2
                     uint32_t A = 0;
                     const uint32_t T = (uint32_t)(((s >> 1) + 3) >> 2);
-                    if (T != 0u) A = WIDE ? scan_dpw((k & 1) ? od_addr : ev_addr, T, h) : scan_dp((k & 1) ? od_addr : ev_addr, T, h);
+                    if (T != 0u) A = WIDE ? scan_dpw((k & 1) ? od_addr : ev_addr, T, h) : scan_dp((k & 1) ? od_addr : ev_addr, T, h, minus1);
                     uint32_t li;                                              // 16 * (b0,b1,bB,bB+1,b2B,b2B+1)
                     if (WIDE) { const uint32_t x = A & 0x00300C03u; li = ((x | (x >> 8) | (x >> 16)) & 0x3Fu) << 4; }
                     else li = (((A & 0x00030303u) * 0x00010410u) >> 12) & 0x3F0u;
