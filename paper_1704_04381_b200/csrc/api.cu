@@ -340,7 +340,7 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
 
     rosen::LatticeParams p{};
     p.N = N; p.n_chains = n_chains; p.chain_offset = chain_offset;
-    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32);
+    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32); p.rk = rosen::philox_round_keys(seed);
     p.ln_shift = ln_shift;
     p.out = st.dev; p.partials = sc->dev; p.vb_counter = sc->vb_counter;
     rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks);

@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(256) lattice_dp_kernel(const LatticeParams p)
 #pragma unroll 2
             for (int q = 0; 4 * q < N; ++q) {
                 uint32_t w[4];
-                philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.key0, p.key1, w);   // L1
+                philox4x32_10(c_lo, c_hi, (uint32_t)q, 0u, p.rk, w);   // L1
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const int s = 4 * q + k;
