@@ -66,7 +66,9 @@ PROFILE_OF = {   # committed ncu summary (profiles/) of the dominant kernel of e
     "lattice_N16_2p16": "r02_lattice_cfg1.md", "lattice_N64_2p24": "r02_lattice_cfg2.md",
     "realspace_N64_k16_2p22": "r02_realspace_cfg3.md", "realspace_N256_k64_2p20_dump": "r02_realspace_cfg5.md",
     "lattice_sweep_N128_2p24": "r02_lattice_sweep_N128.md", "lattice_sweep_N256_2p24": "r02_lattice_sweep_N256.md",
-    "lattice_long_N1024_2p20": "r01e_lattice_long_N1024.md", "realspace_long_N4096_k16_2p16": "r01e_realspace_long_N4096.md",
+    "lattice_long_N1024_2p20": "r02_lattice_long_N1024.md", "lattice_long_N2048_2p19": "r02_lattice_long_N2048.md",
+    "lattice_long_N10000_2p17": "r02_lattice_long_N10000.md", "realspace_long_N4096_k16_2p16": "r02_realspace_long_N4096.md",
+    "realspace_long_N10000_k64_2p14": "r02_realspace_long_N10000.md",
 }
 
 
