@@ -73,6 +73,15 @@ def test_no_cpu_fallback(R):
     rc = lib.rosen_realspace_generate(16, 64, 8, 1.0, 1.0, 1, 0, None, ctypes.byref(summ), None)
     assert rc == R.ROSEN_ECUDA
     assert lib.rosen_lattice_generate(1, 64, 1, 0, None, ctypes.byref(summ), None) == R.ROSEN_EINVAL
+    # the round-2 entry points: model calls, PERM, direction map, store probe -- no CPU path either
+    assert lib.rosen_lattice_generate_model(16, 64, 1, 0, 26, 0.3, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
+    assert lib.rosen_realspace_generate_model(16, 64, 8, 1.0, 1.0, 1.5, 0.3, 1, 0, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
+    thr = (ctypes.c_double * 17)(*([0.0] * 17))
+    assert lib.rosen_lattice_perm(16, 64, 1, 0, thr, thr, 0.0, 1000, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
+    w = (ctypes.c_uint32 * 4)(1, 2, 3, 4)
+    out = (ctypes.c_float * 12)()
+    assert lib.rosen_direction_eval(w, w, 4, out, R.ROSEN_MEM_HOST, None) == R.ROSEN_ECUDA
+    assert lib.rosen_realspace_dump_probe(16, 4, out, None, None) == R.ROSEN_ECUDA
 
 
 def test_product_never_imports_oracle():
