@@ -190,6 +190,56 @@ ROSEN_API int rosen_realspace_generate_async(int32_t N, uint64_t n_chains, int32
                                    const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
 
 /*
+ * rosen_lattice_generate_noalloc -- the lattice call for callers that must not allocate device memory.
+ *
+ * Who needs it: a host program that gave the whole GPU to its own allocator at start-up (a simulation code with one big
+ * arena, a framework whose caching allocator already holds every free byte) finds that a cudaMalloc inside a library
+ * either fails or takes memory the program had budgeted for itself; a service with a fixed, audited memory footprint
+ * may not let a library grow it behind its back; and a loop that must not stall cannot afford cudaMalloc / cudaFree,
+ * which synchronise the whole device. Every other generate call of this header allocates on its first use (block
+ * partials, a pinned summary mirror, events; workspaces for long chains). This one allocates nothing, ever: it makes no
+ * cudaMalloc*, cudaFree*, cudaHostAlloc, stream / event creation or other allocating call, on the first call or later.
+ *
+ * What it computes: exactly rosen_lattice_generate_async (same kernel -- the shared-memory scan kernel of lattice.cu --
+ * same chain ids, same virtual-block partition, same reduction order), so per-chain outputs and every field of the
+ * summary are bit-identical to that call for N < ROSEN_LATTICE_HASH_MIN_N; for longer chains the regular call switches
+ * kernels, and the two agree decision for decision with lnW and the sums within 1e-12, as documented above.
+ *
+ * Where the scratch lives: the kernel's scratch (one 64-byte block partial per virtual block + the virtual-block
+ * ticket) sits in a static __device__ array inside librosen.so, ROSEN_NOALLOC_SCRATCH_BYTES = 512 KiB + 256 B. The
+ * CUDA runtime places it on every GPU on which the process uses this library, and it stays there until the process
+ * exits; that is the whole price.
+ *
+ * Limits: 2 <= N <= ROSEN_NOALLOC_MAX_N (the scan kernel's range; longer chains need gigabytes of hash tables, which
+ * no static array can hold) and 1 <= n_chains <= ROSEN_NOALLOC_MAX_CHAINS per call (one partial per 2048 chains fills
+ * the array). Anything beyond returns ROSEN_ERANGE with a message naming the limit and launches nothing; cover a
+ * larger population with several calls over consecutive chain_offset ranges and merge the summaries with
+ * rosen_summary_merge (bit-identical per chain; that is what the ids are for).
+ *
+ * Arguments: outputs (may be NULL) must hold DEVICE pointers only (memory == ROSEN_MEM_DEVICE, else ROSEN_EINVAL: a
+ * host destination would need a staging allocation). summary_device (may be NULL) is a DEVICE pointer to
+ * sizeof(rosen_summary) caller-owned bytes, 8-byte aligned, filled on cuda_stream, derived fields included; copy it
+ * out yourself. The call only enqueues work (one cudaMemsetAsync of the 4-byte ticket, the generation kernel, and the
+ * second reduction pass when summary_device is set) and returns; nothing is synchronised.
+ *
+ * First call on each device: it looks up the device address of the static array (cudaGetSymbolAddress, with that device
+ * current) and remembers it; this is also when the CUDA runtime loads the library's kernels onto that device. Make that
+ * first call during start-up, outside any stream capture; later calls on the device do no set-up at all.
+ *
+ * Sharing: all no-allocation calls on a device use the SAME array. The ticket is re-zeroed on the stream by every call
+ * and every partial the second pass reads is rewritten by the kernel first, so a call never sees what the previous one
+ * left behind -- provided the calls do not overlap on the GPU. Two such calls in flight at once on one device (different
+ * streams without an event between them) race on the array and give wrong sums: keep them on one stream or order them
+ * yourself; the library takes no lock and records no event here, since creating one would allocate. The array is
+ * private to this entry point, so these calls do not disturb, and are not disturbed by, the other calls of this header.
+ */
+#define ROSEN_NOALLOC_MAX_N         ROSEN_LATTICE_SCAN_MAX_N
+#define ROSEN_NOALLOC_MAX_CHAINS    (1ull << 24)
+#define ROSEN_NOALLOC_SCRATCH_BYTES (8192 * 64 + 256)
+ROSEN_API int rosen_lattice_generate_noalloc(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream);
+
+/*
  * The direction map "rngonsphere" of Alg. 2 line 10 (reading A10) alone, as the real-space
  * kernels evaluate it: dir_xyz[3 i .. 3 i + 2] = unit vector of the Philox word pair (wz[i], wphi[i]). A component of
  * step R1 exposed so that parity tests can sweep it exhaustively (all 2^23 polar values; every azimuth octant) against

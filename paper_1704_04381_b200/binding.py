@@ -73,6 +73,8 @@ def load_library() -> C.CDLL:
     L.rosen_realspace_generate_async.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64,
                                                  C.POINTER(rosen_outputs), vp, vp]
     L.rosen_realspace_generate_async.restype = C.c_int
+    L.rosen_lattice_generate_noalloc.argtypes = [i32, u64, u64, u64, C.POINTER(rosen_outputs), vp, vp]
+    L.rosen_lattice_generate_noalloc.restype = C.c_int
     L.rosen_lattice_dump.argtypes = [i32, u64, u64, u64, vp, vp, i32, C.POINTER(rosen_summary), vp]
     L.rosen_lattice_dump.restype = C.c_int
     L.rosen_realspace_dump.argtypes = [i32, u64, i32, C.c_float, C.c_float, u64, u64, vp, vp, i32,
@@ -264,6 +266,24 @@ def rosen_lattice_generate_async(N: int, n_chains: int, seed: int, chain_offset:
     _check(L.rosen_lattice_generate_async(N, n_chains, seed, chain_offset, C.byref(st),
                                           summary_device.data_ptr() if summary_device is not None else None,
                                           _stream_ptr(stream)))
+
+
+ROSEN_NOALLOC_MAX_N, ROSEN_NOALLOC_MAX_CHAINS, ROSEN_NOALLOC_SCRATCH_BYTES = 512, 1 << 24, 8192 * 64 + 256
+
+
+def rosen_lattice_generate_noalloc(N: int, n_chains: int, seed: int, chain_offset: int = 0, outputs=None,
+                                   summary_device=None, stream=None) -> None:
+    """rosen_lattice_generate_noalloc of include/rosen.h: the lattice call for programs that cannot let a library
+    allocate GPU memory (their own allocator owns the device, or their footprint is fixed, or they cannot afford the
+    device-wide stall of cudaMalloc). Enqueue only, and this wrapper allocates nothing either: outputs = {name: CUDA
+    tensor the caller made}, summary_device = a uint8 CUDA tensor of SUMMARY_BYTES (8-byte aligned) the caller made, or
+    None. N <= ROSEN_NOALLOC_MAX_N and n_chains <= ROSEN_NOALLOC_MAX_CHAINS, else RosenError(ROSEN_ERANGE). Calls
+    on one device share one static scratch array: do not let two of them overlap on the GPU."""
+    L = load_library()
+    st = _outputs_struct(outputs)
+    _check(L.rosen_lattice_generate_noalloc(N, n_chains, seed, chain_offset, C.byref(st),
+                                            summary_device.data_ptr() if summary_device is not None else None,
+                                            _stream_ptr(stream)))
 
 
 def rosen_realspace_generate_async(N: int, n_chains: int, k_trials: int, bond_len: float, sigma: float, seed: int,

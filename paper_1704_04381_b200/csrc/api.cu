@@ -595,6 +595,88 @@ int perm_impl(int32_t N, uint64_t n_tours, uint64_t seed, uint64_t tour_offset, 
     return finish(sc, (int)pp.n_vblocks, n_tours, 0.0, pp.lmax + rosen::kMaxPartials, outputs, zs, st, summary, nullptr, stream);
 }
 
+// ---- rosen_lattice_generate_noalloc: the lattice scan kernel with its scratch in static device memory ----------------
+// For callers that may not allocate (rosen.h says who and why). Nothing below calls cudaMalloc*, cudaFree*, cudaHostAlloc,
+// or creates a stream or an event, and it does not touch the Scratch of the other entry points (get_scratch allocates).
+//
+// Layout of the array: [0, kNoAllocPartialBytes) block partials, one per virtual block; then the 4-byte virtual-block
+// ticket in a 256-byte slot of its own, so that the memset of the ticket never shares a line with a partial.
+constexpr size_t kNoAllocPartialBytes = sizeof(Partial) * rosen::kMaxPartials;
+static_assert(kNoAllocPartialBytes + 256 == ROSEN_NOALLOC_SCRATCH_BYTES, "rosen.h states the size of the static scratch");
+static_assert(ROSEN_NOALLOC_MAX_CHAINS == (uint64_t)rosen::kMaxPartials * rosen::kMinChunk, "one partial per kMinChunk chains");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[ROSEN_NOALLOC_SCRATCH_BYTES];
+
+// In host code `g_noalloc_scratch` is only a handle for the runtime's symbol table, NOT a device address: handing it to a
+// kernel would fault (or, on a machine where the GPU can read host memory, quietly use the wrong memory). The address is
+// asked for once per device, with that device current, and cached here.
+unsigned char* g_noalloc_addr[kMaxDevices] = {};
+std::mutex g_noalloc_mutex;
+
+int noalloc_scratch(unsigned char** out)
+{
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) { std::snprintf(g_err, sizeof(g_err), "device index %d unsupported", dev); return ROSEN_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[dev]) {
+        void* addr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&addr, g_noalloc_scratch);
+        if (e != cudaSuccess || !addr) return fail_cuda(e != cudaSuccess ? e : cudaErrorInvalidSymbol, "cudaGetSymbolAddress(static scratch)");
+        g_noalloc_addr[dev] = static_cast<unsigned char*>(addr);
+    }
+    *out = g_noalloc_addr[dev];
+    return ROSEN_OK;
+}
+
+int lattice_noalloc_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, const rosen_outputs* outputs,
+                         rosen_summary* summary_dev, void* cuda_stream)
+{
+    g_err[0] = 0; g_launches = 0; g_kernel = "";
+    if (N < 2 || n_chains == 0) { std::snprintf(g_err, sizeof(g_err), "need N >= 2 and n_chains >= 1"); return ROSEN_EINVAL; }
+    if (outputs && outputs->memory != ROSEN_MEM_DEVICE) {
+        std::snprintf(g_err, sizeof(g_err), "rosen_lattice_generate_noalloc takes device outputs only (a host destination needs a staging allocation)");
+        return ROSEN_EINVAL;
+    }
+    if (N > ROSEN_NOALLOC_MAX_N) {
+        std::snprintf(g_err, sizeof(g_err), "rosen_lattice_generate_noalloc: N = %d exceeds ROSEN_NOALLOC_MAX_N = %d (longer chains need the "
+                      "allocating rosen_lattice_generate)", N, ROSEN_NOALLOC_MAX_N);
+        return ROSEN_ERANGE;
+    }
+    if (n_chains > ROSEN_NOALLOC_MAX_CHAINS) {
+        std::snprintf(g_err, sizeof(g_err), "rosen_lattice_generate_noalloc: n_chains = %llu exceeds ROSEN_NOALLOC_MAX_CHAINS = %llu, the capacity of the "
+                      "static scratch (split the range over several calls with chain_offset)",
+                      (unsigned long long)n_chains, (unsigned long long)ROSEN_NOALLOC_MAX_CHAINS);
+        return ROSEN_ERANGE;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    unsigned char* scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc) return rc;
+
+    rosen::LatticeParams p{};
+    p.N = N; p.n_chains = n_chains; p.chain_offset = chain_offset;
+    p.key0 = (uint32_t)seed; p.key1 = (uint32_t)(seed >> 32); p.rk = rosen::philox_round_keys(seed);
+    p.ln_shift = std::log(6.0) + (double)(N - 2) * std::log(5.0);
+    if (outputs) p.out = DevOutputs{outputs->lnW, outputs->alive, outputs->m_seq, outputs->digest, outputs->conf, outputs->ree2, outputs->rg2};
+    p.partials = reinterpret_cast<Partial*>(scratch);
+    p.vb_counter = reinterpret_cast<uint32_t*>(scratch + kNoAllocPartialBytes);
+    rosen::partition_chains(n_chains, &p.chunk, &p.n_vblocks);          // the regular call's partition: same sums, bit for bit
+    if (p.n_vblocks > (uint32_t)rosen::kMaxPartials) { std::snprintf(g_err, sizeof(g_err), "static scratch too small for %u virtual blocks", p.n_vblocks); return ROSEN_ERANGE; }
+    // the array keeps whatever the last call left: the ticket must start at 0; partials [0, n_vblocks) are all rewritten by
+    // the kernel before the second pass reads them, the rest is never read
+    CK(cudaMemsetAsync(p.vb_counter, 0, sizeof(uint32_t), stream));
+    int grid = 0;
+    rc = rosen::launch_lattice(p, stream, &g_kernel, &grid);
+    if (rc < 0) return rc == -2 ? ROSEN_ERANGE : fail_cuda(cudaGetLastError(), "lattice kernel launch");
+    g_launches += rc;
+    if (summary_dev) {
+        if (rosen::launch_finalize(p.partials, (int)p.n_vblocks, n_chains, p.ln_shift, nullptr, summary_dev, stream) < 0)
+            return fail_cuda(cudaGetLastError(), "finalize_kernel");
+        ++g_launches;
+    }
+    return ROSEN_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -629,6 +711,12 @@ int rosen_realspace_generate_async(int32_t N, uint64_t n_chains, int32_t k_trial
         std::snprintf(g_err, sizeof(g_err), "the _async calls take device outputs only"); return ROSEN_EINVAL;
     }
     return realspace_impl(N, n_chains, k_trials, bond_len, sigma, seed, chain_offset, outputs, nullptr, summary_device, cuda_stream);
+}
+
+int rosen_lattice_generate_noalloc(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
+                                   const rosen_outputs* outputs, rosen_summary* summary_device, void* cuda_stream)
+{
+    return lattice_noalloc_impl(N, n_chains, seed, chain_offset, outputs, summary_device, cuda_stream);
 }
 
 int rosen_lattice_dump(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,

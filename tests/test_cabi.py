@@ -27,7 +27,7 @@ def declared_symbols():
 def test_every_declared_symbol_is_exported(R):
     from paper_1704_04381_b200 import binding
     names = declared_symbols()
-    assert len(names) == 20 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
+    assert len(names) == 21 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
     lib = ctypes.CDLL(binding.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), n
@@ -75,6 +75,7 @@ def test_no_cpu_fallback(R):
     assert lib.rosen_lattice_generate(1, 64, 1, 0, None, ctypes.byref(summ), None) == R.ROSEN_EINVAL
     # the round-2 entry points: model calls, PERM, direction map, store probe -- no CPU path either
     assert lib.rosen_lattice_generate_model(16, 64, 1, 0, 26, 0.3, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
+    assert lib.rosen_lattice_generate_noalloc(16, 64, 1, 0, None, None, None) == R.ROSEN_ECUDA
     assert lib.rosen_realspace_generate_model(16, 64, 8, 1.0, 1.0, 1.5, 0.3, 1, 0, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
     thr = (ctypes.c_double * 17)(*([0.0] * 17))
     assert lib.rosen_lattice_perm(16, 64, 1, 0, thr, thr, 0.0, 1000, None, ctypes.byref(summ), None) == R.ROSEN_ECUDA
