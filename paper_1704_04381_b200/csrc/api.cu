@@ -411,7 +411,10 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
             if (rc) return rc;
             if ((rc = grow(&sc->hash_rec, &sc->hash_rec_bytes, n_chains * sizeof(rosen::ChainRecord)))) return rc;
             if (!sc->hash_ticket) CK(cudaMalloc(&sc->hash_ticket, sizeof(unsigned long long)));
-            const uint64_t layout = (2ull << 62) | ((uint64_t)(lp.warp_bytes >> 8) << 24) | (uint64_t)warps;
+            // the key holds what fixes every table's byte offset: n_pad (where the cell table starts inside a warp's slice), entries and
+            // the warp count. The rounded warp_bytes alone would let N = 1000 (n_pad 1000) reuse the tables of N = 1001 (n_pad 1008,
+            // same 32256-byte slice), whose chain slots 1000..1007 would then be read as cell entries.
+            const uint64_t layout = (2ull << 62) | ((uint64_t)lp.n_pad << 44) | ((uint64_t)lp.entries << 24) | (uint64_t)warps;
             if ((rc = prepare_workspace(sc, layout, warps * lp.warp_bytes, sc->hash_tables_bytes != had, stream))) return rc;
         }
         lp.gen_store = sc->hash_gen;

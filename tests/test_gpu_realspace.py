@@ -104,6 +104,15 @@ def test_long_chains_cell_list_kernel(R, N, n, k, b, sigma, seed, offset):
     assert "realspace_long_kernel" in R.rosen_last_kernel_name() and R.rosen_last_launch_count() == 5
 
 
+def test_cell_list_workspace_reuse_across_neighbouring_lengths(R):
+    """N = 1000 (n_pad 1000) and N = 1001 (n_pad 1008) round to the same 32256-byte slice per warp but put the cell table at
+    different offsets: the workspace must be cleared between them (its layout key holds n_pad and entries, not the rounded
+    slice size), or the shorter call would read the longer call's last chain slots as cell entries."""
+    for N, seed in [(1001, 31), (1000, 32), (1001, 33), (1000, 34), (1007, 35), (1000, 31)]:
+        check(R, N, 24, 16, 1.0, 0.6, seed, 0)
+        assert "realspace_long_kernel" in R.rosen_last_kernel_name()
+
+
 @pytest.mark.parametrize("cap", [None, "33"])
 def test_cell_list_kernel_on_short_chains(R, monkeypatch, cap):
     """ROSEN_REALSPACE_CELL_MIN_N routes short chains through the cell-list kernel, where the oracle's full scan is
