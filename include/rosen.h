@@ -21,8 +21,9 @@
  *     multi-GPU sharding, resume and sampled parity checks work.
  *   - Calls on one device share that device's scratch (block partials; the long-chain workspace). The library keeps them
  *     apart itself: host threads are serialised per device for the duration of a call, and a call enqueued on another
- *     stream than the previous call of that device first waits (cudaStreamWaitEvent) for that call's work. Calls on
- *     different devices are independent.
+ *     stream than the previous call of that device first waits (cudaStreamWaitEvent) for that call's work; this holds for
+ *     the _async calls too, which are thereby ordered across streams on the device. Calls on different devices are
+ *     independent.
  *   - There is no CPU fallback: without a CUDA device every generate call fails with ROSEN_ECUDA.
  */
 #ifndef ROSEN_H
@@ -107,9 +108,8 @@ typedef struct rosen_outputs {
  * chain (W = 0, kept). 2 <= N <= ROSEN_LATTICE_MAX_N. For N >= ROSEN_LATTICE_HASH_MIN_N the library keeps device
  * workspace (at most 12 GiB of per-chain hash tables + 40 bytes per chain of the largest call) until
  * rosen_workspace_release(); decisions (trajectory, m sequence, digest) do not depend on which kernel ran, lnW and the sums agree to 1e-12
- * (different rounding order). The tables are cleared only when they are allocated or their layout changes. That workspace is one per device:
- * long-chain calls (lattice or real space) on the same device must not overlap in time, i.e. enqueue them on one stream
- * or synchronise between streams / host threads.
+ * (different rounding order). The tables are cleared only when they are allocated or their layout changes. That workspace is one per
+ * device; the library keeps the calls that share it apart itself (see Conventions above).
  */
 ROSEN_API int rosen_lattice_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset,
                            const rosen_outputs* outputs, rosen_summary* summary, void* cuda_stream);
@@ -261,13 +261,6 @@ ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trial
                          float* conf, double* lnW, int32_t memory, rosen_summary* summary, void* cuda_stream);
 
 /*
- * Merge the summaries of disjoint chain ranges generated with the same (N, k_trials) -- the only
- * "exchange" a multi-GPU run needs (DESIGN.md 7). Sums are added in array order (deterministic),
- * derived fields recomputed. Parts with different ln_shift (long chains) are rescaled to the largest shift of a
- * part with sum_w > 0. Returns ROSEN_EINVAL if count == 0 or a shift is not finite.
- * Pure host function.
- */
-/*
  * The store phase of rosen_realspace_dump ALONE ("HBM GB/s is only meaningful for the store phase
  * measured alone ... a dump-only kernel"): every lane group keeps one synthetic chain (r_i = (i, i/2, -i)) resident in
  * shared memory and stores it to conf[c][N][3] (and (double)c to lnW[c], if non-NULL) for every chain c < n_chains, with
@@ -276,6 +269,13 @@ ROSEN_API int rosen_realspace_dump(int32_t N, uint64_t n_chains, int32_t k_trial
  */
 ROSEN_API int rosen_realspace_dump_probe(int32_t N, uint64_t n_chains, float* conf, double* lnW, void* cuda_stream);
 
+/*
+ * Merge the summaries of disjoint chain ranges generated with the same (N, k_trials) -- the only
+ * "exchange" a multi-GPU run needs (DESIGN.md 7). Sums are added in array order (deterministic),
+ * derived fields recomputed. Parts with different ln_shift (long chains) are rescaled to the largest shift of a
+ * part with sum_w > 0. Returns ROSEN_EINVAL if count == 0 or a shift is not finite.
+ * Pure host function.
+ */
 ROSEN_API int rosen_summary_merge(const rosen_summary* parts, int32_t count, rosen_summary* merged);
 
 /*
@@ -297,12 +297,19 @@ typedef struct rosen_fit {
 ROSEN_API int rosen_fit_exponents(const int32_t* N, const double* mean_ree2, const double* ln_mean_W,
                                   int32_t count, int32_t use_steps, rosen_fit* fit);
 
-/* Bytes of device scratch the library currently keeps on the current device: block partials, plus the
- * long-chain workspace of the lattice call if one was made (informational). */
+/* Bytes of device memory the library currently keeps on the current device (informational): block partials and the summary
+ * slot (always), plus whatever the calls made so far left behind -- the long-chain tables (at most 12 GiB) with their
+ * generation counters (4 MiB), 40 bytes per chain of the largest long-chain / model / PERM call, the PERM thresholds (8 KiB).
+ * Not counted: staging buffers of ROSEN_MEM_HOST calls. Those are stream-ordered allocations from the device's DEFAULT memory
+ * pool, whose release threshold the library raises on first use so that freed staging memory (3.2 GB at BASELINE config 5)
+ * stays in the pool for the next call instead of going back to the driver at every synchronisation; other users of
+ * cudaMalloc on the device do not see that memory as free until rosen_workspace_release() trims the pool. */
 ROSEN_API size_t rosen_workspace_bytes(void);
 
-/* Free the long-chain workspace of the current device (synchronises the device). Always ROSEN_OK; the next
- * long-chain call allocates it again. */
+/* Free what the calls on the current device left behind: the long-chain / model / PERM workspace, the mapped flags, copy
+ * stream and ordering event of earlier calls, and the unused part of the default memory pool (cudaMemPoolTrimTo 0). Waits for
+ * calls of other host threads on this device to return, then synchronises the device. Always ROSEN_OK; later calls allocate
+ * again what they need. */
 ROSEN_API int rosen_workspace_release(void);
 
 /*

@@ -49,13 +49,13 @@ struct Scratch {
     cudaStream_t   copy_stream = nullptr;  // device->host copies of finished conformations while the kernel runs
     uint32_t*      hash_gen = nullptr;     // [kMaxGenSlots] generation counters of the long-chain kernels' threads / warps
     uint64_t       ws_layout = 0;          // signature of the table layout the workspace was last cleared for (0: none)
-    double*        perm_thr = nullptr;
+    double*        perm_thr = nullptr;    // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
     // calls of one device share everything above: host threads take call_mutex for the whole call, and a call on another
     // stream than the previous one first waits for that call's last enqueued work (last_done)
     std::mutex     call_mutex;
     cudaEvent_t    last_done = nullptr;
     cudaStream_t   last_stream = nullptr;
-    bool           have_last = false;     // [2][ROSEN_PERM_MAX_N + 1] PERM thresholds (ln_lo | ln_hi)
+    bool           have_last = false;
 };
 constexpr size_t kHashTableCap = (size_t)12 << 30;  // bytes of per-chain hash tables kept resident at most
 constexpr int kMaxDevices = 64;
@@ -101,7 +101,9 @@ int CallGuard::enter(Scratch* s, cudaStream_t st)
     s->call_mutex.lock();
     sc = s; stream = st;
     if (!s->last_done) CK(cudaEventCreateWithFlags(&s->last_done, cudaEventDisableTiming));
-    if (s->have_last && s->last_stream != st) CK(cudaStreamWaitEvent(st, s->last_done, 0));
+    // always wait, even when the handle equals the previous call's: a caller may have destroyed that stream with work pending and
+    // been handed the same handle value for a new one; waiting on an event of the same stream costs next to nothing
+    if (s->have_last) CK(cudaStreamWaitEvent(st, s->last_done, 0));
     return ROSEN_OK;
 }
 CallGuard::~CallGuard()
@@ -139,7 +141,7 @@ int prepare_workspace(Scratch* sc, uint64_t layout, size_t table_bytes_total, bo
 // Host conformation buffers (ROSEN_MEM_HOST + conf): the generation kernel raises a flag in mapped host memory for every
 // virtual block whose outputs are stored; this loop copies the finished chain ranges device -> host on a second stream while
 // the kernel is still running, so the PCIe transfer of the dump (3.2 GB at config 5) overlaps the generation instead of following it.
-int stream_conf_out(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, void* conf_host, size_t row_bytes,
+int stream_conf_out_loop(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, void* conf_host, size_t row_bytes,
                     uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks)
 {
     volatile uint32_t* flags = sc->done_flags;
@@ -160,8 +162,19 @@ int stream_conf_out(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, 
         if (q == cudaSuccess) { kernel_over = true; continue; }           // one more pass over the flags
         if (q != cudaErrorNotReady) return fail_cuda(q, "generation kernel");
     }
-    CK(cudaStreamSynchronize(sc->copy_stream));
     if (next < n_vblocks) { std::snprintf(g_err, sizeof(g_err), "generation kernel ended without storing every virtual block"); return ROSEN_ECUDA; }
+    return ROSEN_OK;
+}
+
+int stream_conf_out(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, void* conf_host, size_t row_bytes,
+                    uint64_t n_chains, uint32_t chunk, uint32_t n_vblocks)
+{
+    const int rc = stream_conf_out_loop(sc, gen_stream, conf_dev, conf_host, row_bytes, n_chains, chunk, n_vblocks);
+    // on success and on every error path: the copy stream has finished reading the staging buffer before the caller's
+    // ~Staging hands it back to the pool on the generation stream
+    const cudaError_t e = cudaStreamSynchronize(sc->copy_stream);
+    if (rc) { cudaGetLastError(); return rc; }
+    if (e != cudaSuccess) return fail_cuda(e, "cudaStreamSynchronize(copy stream)");
     return ROSEN_OK;
 }
 
@@ -872,7 +885,10 @@ size_t rosen_workspace_bytes(void)
     int dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices) {
         std::lock_guard<std::mutex> lock(g_mutex);
-        b += g_scratch[dev].hash_tables_bytes + g_scratch[dev].hash_rec_bytes;
+        const Scratch& s = g_scratch[dev];
+        b += s.hash_tables_bytes + s.hash_rec_bytes;
+        if (s.hash_gen) b += kMaxGenSlots * sizeof(uint32_t);
+        if (s.perm_thr) b += sizeof(double) * 2 * (ROSEN_PERM_MAX_N + 1);
     } else {
         cudaGetLastError();
     }
@@ -883,15 +899,31 @@ int rosen_workspace_release(void)
 {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return ROSEN_OK; }   // nothing was ever allocated
-    std::lock_guard<std::mutex> lock(g_mutex);
     Scratch& s = g_scratch[dev];
-    if (s.hash_tables || s.hash_rec || s.hash_ticket) cudaDeviceSynchronize();
+    // call_mutex first, then g_mutex: the order the generate calls use. A call of another host thread that has already read
+    // the workspace pointers into its kernel parameters finishes enqueueing before anything is freed; the device
+    // synchronisation below then waits for that work.
+    std::lock_guard<std::mutex> call_lock(s.call_mutex);
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (s.dev) cudaDeviceSynchronize();                 // s.dev: some call has used this device
     if (s.hash_tables) { cudaFree(s.hash_tables); s.hash_tables = nullptr; s.hash_tables_bytes = 0; }
     if (s.hash_gen) { cudaFree(s.hash_gen); s.hash_gen = nullptr; }
     s.ws_layout = 0;
     if (s.hash_rec) { cudaFree(s.hash_rec); s.hash_rec = nullptr; s.hash_rec_bytes = 0; }
     if (s.hash_ticket) { cudaFree(s.hash_ticket); s.hash_ticket = nullptr; }
     if (s.perm_thr) { cudaFree(s.perm_thr); s.perm_thr = nullptr; }
+    // what the host-dump overlap and the cross-stream ordering created on demand; the next call that needs them makes them again
+    if (s.done_flags) { cudaFreeHost(s.done_flags); s.done_flags = nullptr; }
+    if (s.copy_stream) { cudaStreamDestroy(s.copy_stream); s.copy_stream = nullptr; }
+    if (s.last_done) { cudaEventDestroy(s.last_done); s.last_done = nullptr; }
+    s.have_last = false; s.last_stream = nullptr;       // the device is idle: nothing left to order against
+    // staging memory of host-pointer calls stays in the device's default memory pool (get_scratch raises its release
+    // threshold so that gigabytes are not returned to the driver at every synchronisation): hand the unused part back now
+    if (s.dev) {
+        cudaMemPool_t pool = nullptr;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) cudaMemPoolTrimTo(pool, 0);
+    }
+    cudaGetLastError();
     return ROSEN_OK;
 }
 int32_t rosen_last_launch_count(void) { return g_launches; }

@@ -317,3 +317,38 @@ def test_concurrent_calls_from_threads_and_streams(R):
     for t in th: t.join()
     for (s0, t0), (s1, t1) in zip(want, got):
         assert s0 == s1 and torch.equal(t0["digest"], t1["digest"])
+
+
+def test_workspace_release_while_other_threads_call(R):
+    """rosen_workspace_release takes the same per-device lock as the generate calls: a release issued while another host
+    thread is inside a long-chain / model call waits for that call instead of freeing the tables its kernel is about to use."""
+    import threading
+    import torch
+    jobs = [(300, 3000, 300), (1024, 500, 301)]
+    want = [R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW")) for N, n, seed in jobs]
+    got = [[] for _ in jobs]
+    stop = threading.Event()
+
+    def run(i):
+        N, n, seed = jobs[i]
+        st = torch.cuda.Stream()
+        for _ in range(12):
+            got[i].append(R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW"), stream=st))
+
+    def release():
+        while not stop.is_set():
+            assert R.rosen_workspace_release() == R.ROSEN_OK
+
+    th = [threading.Thread(target=run, args=(i,)) for i in range(len(jobs))]
+    rel = threading.Thread(target=release)
+    rel.start()
+    for t in th: t.start()
+    for t in th: t.join()
+    stop.set(); rel.join()
+    for (s0, t0), runs in zip(want, got):
+        assert len(runs) == 12
+        for s1, t1 in runs:
+            assert s0 == s1 and torch.equal(t0["digest"], t1["digest"]) and torch.equal(t0["lnW"], t1["lnW"])
+    assert R.rosen_workspace_release() == R.ROSEN_OK
+    s2, t2 = R.rosen_lattice_generate(*jobs[1], outputs=("digest", "lnW"))       # everything released is made again
+    assert s2 == want[1][0] and torch.equal(t2["digest"], want[1][1]["digest"])
