@@ -58,6 +58,8 @@ def lib() -> C.CDLL:
         L.oracle_saw_enumerate.restype = C.c_int
         L.oracle_model_table.argtypes = [C.c_double, C.POINTER(C.c_uint64)]
         L.oracle_model_table.restype = None
+        L.oracle_scaled_target.argtypes = [C.c_uint32, C.c_uint64]
+        L.oracle_scaled_target.restype = C.c_uint64
         L.oracle_lattice_model_step.argtypes = [C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.POINTER(C.c_uint64),
                                                 C.POINTER(C.c_uint64)]
         L.oracle_lattice_model_step.restype = C.c_int32
@@ -159,6 +161,11 @@ def model_table(beta_eps: float) -> list:
     q = (C.c_uint64 * 32)()
     lib().oracle_model_table(beta_eps, q)
     return [int(v) for v in q]
+
+
+def scaled_target(u: int, W: int) -> int:
+    """floor(u W / 2^32) as the model oracles compute it (the threshold of the Boltzmann-proportional choice)."""
+    return int(lib().oracle_scaled_target(u, W))
 
 
 def lattice_model_step(r: np.ndarray, z: int, beta_eps: float) -> list:

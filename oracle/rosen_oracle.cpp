@@ -447,6 +447,9 @@ static uint64_t scaled_target(uint32_t u, uint64_t W)
     return (W >> 32) * (uint64_t)u + (((W & 0xFFFFFFFFull) * (uint64_t)u) >> 32);
 }
 
+// the same routine, exported so that a test can pin it against Python's big integers: (u W) >> 32
+uint64_t oracle_scaled_target(uint32_t u, uint64_t W) { return scaled_target(u, W); }
+
 int oracle_lattice_model_generate(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_offset, int32_t z,
                                   double beta_eps, const oracle_outputs* out, oracle_summary* summary)
 {

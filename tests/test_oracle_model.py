@@ -151,3 +151,51 @@ def test_realspace_beta0_reproduces_base_and_well_counts():
     expect = (1 - p_well) + q * (p_well - p_core)
     se = W.std(ddof=1) / math.sqrt(len(W))
     assert abs(W.mean() - expect) < 5 * se + 1e-4, (W.mean(), expect, se)
+
+
+def test_scaled_target_is_the_big_integer_quotient():
+    """floor(u W / 2^32) (the selection threshold) against Python's exact integers, over both branches of
+    the two-limb product: W < 2^32 (every z = 6 step) and W >= 2^32 (reached at z = 26, beta eps near 0.85), the carries
+    at the limb boundary, and the extremes. A dropped high limb, a wrong shift or a missing carry fails here."""
+    rng = np.random.default_rng(17)
+    us = [0, 1, 2, 0x7FFFFFFF, 0x80000000, 0xFFFFFFFE, 0xFFFFFFFF] + [int(v) for v in rng.integers(0, 1 << 32, 200)]
+    Ws = [1, 2, 65536, 6 * 65536, (1 << 32) - 1, 1 << 32, (1 << 32) + 1, (1 << 33) - 1, 0x1_0000_FFFF, 0xFFFF_FFFF_FFFF,
+          (1 << 62) + 12345, (1 << 63) - 1] + [int(v) for v in rng.integers(1, 1 << 62, 200)] \
+         + [int(v) for v in rng.integers(1, 1 << 34, 200)]
+    for u in us:
+        for W in Ws:
+            assert oracle.scaled_target(u, W) == (u * W) >> 32, (u, W)
+    # the largest W a step can have: 26 free trials of 25 contacts each at beta eps = 0.85
+    W = 26 * oracle.model_table(0.85)[25]
+    assert W >= 1 << 32 and oracle.scaled_target(0xFFFFFFFF, W) == (0xFFFFFFFF * W) >> 32 < W
+
+
+@pytest.mark.parametrize("k,seed", [(2, 41), (5, 42), (64, 43)])
+def test_realspace_well_choice_is_boltzmann_proportional(k, seed):
+    """Pins the CHOICE of oracle_realspace_model_generate (a trial is taken with probability Q[c_t] / W_s, Eq. 1-2
+    PAPER.md:47-52), which the E[W] pin above cannot see. N = 3, b = 1: the bond-angle cosine c is uniform on [-1, 1] and
+    Ree2 = 2 (1 + c); with t = 1 + c a trial overlaps for t < a = sigma^2 / 2 and sits in the well for t < w =
+    (lambda sigma)^2 / 2, so the Boltzmann mean over the allowed directions is
+        <Ree2> = [q (w^2 - a^2) + (4 - w^2)] / [q (w - a) + (2 - w)],  q = exp(beta eps),
+    and the Rosenbluth estimator E[W Ree2] / E[W] equals it for ANY k when the choice is proportional to the weights.
+    A uniform choice among the free trials gives something else (for large k: (4 - a^2) / (2 - a) = 2.5, the hard-sphere
+    value), as does a choice by 1/weight or an off-by-one in the cumulative scan. The 2^-16 fixed point moves it by < 1e-5."""
+    sigma, lam, beta = 1.0, 1.5, 0.6
+    q = math.exp(beta)
+    a, w = sigma ** 2 / 2, (lam * sigma) ** 2 / 2
+    exact = (q * (w * w - a * a) + (4 - w * w)) / (q * (w - a) + (2 - w))
+    assert math.isclose(exact, (1.015625 * q + 2.734375) / (0.625 * q + 0.875), rel_tol=1e-15) and abs(exact - 2.2767) < 1e-4
+    M = 150000
+    o = oracle.realspace_model_generate(3, M, k, 1.0, sigma, lam, beta, seed, outputs=("lnW", "ree2", "alive"))
+    W = np.where(o.alive.astype(bool), np.exp(o.lnW), 0.0)
+    est = (W * o.ree2).sum() / W.sum()
+    se = math.sqrt(((W * (o.ree2 - est)) ** 2).sum()) / W.sum()          # delta method
+    assert se < 0.01 and abs(est - exact) < 5 * se + 1e-4, (k, est, exact, se)
+    assert abs(est - 2.5) > 10 * se                                       # the hard-sphere mean is resolved and excluded
+    assert math.isclose(o.summary["mean_ree2"], est, rel_tol=1e-9)
+    # q = 1 gives back the hard-sphere closed form 2.5 (survey pin P5) through the same code path
+    o0 = oracle.realspace_model_generate(3, M, k, 1.0, sigma, lam, 0.0, seed, outputs=("lnW", "ree2", "alive"))
+    W0 = np.where(o0.alive.astype(bool), np.exp(o0.lnW), 0.0)
+    est0 = (W0 * o0.ree2).sum() / W0.sum()
+    se0 = math.sqrt(((W0 * (o0.ree2 - est0)) ** 2).sum()) / W0.sum()
+    assert abs(est0 - 2.5) < 5 * se0 + 1e-4, (est0, se0)
