@@ -56,3 +56,31 @@ def oracle_population(kind: str, N: int, n_chains: int, seed: int, k=None, b=Non
     m["ln_mean_W"] = L + math.log(m["sum_w"] / m["n_chains"])
     arrays = {name: np.concatenate([getattr(p, name) for p in parts]) for name in outputs}
     return m, arrays
+
+
+def oracle_workload_arrays(w, n_chains: int, want=("digest",), ranges_per_thread: int = 8):
+    """Per-chain arrays (and the exact integer totals) of a model / PERM workload (paper_1704_04381_b200.workloads.Workload
+    with beta_eps or perm set) over chain / tour ids 0..n_chains-1. These calls shift their sums by the largest lnW of the
+    CALL, so sub-range summaries do not merge by addition: whole populations are compared chain by chain instead."""
+    from paper_1704_04381_b200 import workloads
+    threads = host_threads()
+    n_ranges = max(1, min(n_chains, threads * ranges_per_thread))
+    bounds = [(n_chains * i) // n_ranges for i in range(n_ranges + 1)]
+    outputs = tuple(want)
+    if w.perm is not None:
+        lo_thr, hi_thr, ref = workloads.perm_thresholds(w.N, *w.perm)
+
+    def one(i):
+        lo, cnt = bounds[i], bounds[i + 1] - bounds[i]
+        if w.perm is not None:
+            return oracle.lattice_perm(w.N, cnt, w.seed, lo_thr, hi_thr, ref, tour_offset=lo, outputs=outputs)
+        if w.kind == "lattice":
+            return oracle.lattice_model_generate(w.N, cnt, w.seed, z=w.z, beta_eps=w.beta_eps, chain_offset=lo, outputs=outputs)
+        return oracle.realspace_model_generate(w.N, cnt, w.k_trials, w.bond_len, w.sigma, w.lam, w.beta_eps, w.seed,
+                                               chain_offset=lo, outputs=outputs)
+
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        parts = list(ex.map(one, range(n_ranges)))
+    totals = {key: sum(p.summary[key] for p in parts) for key in INT_KEYS}
+    arrays = {name: np.concatenate([getattr(p, name) for p in parts]) for name in outputs}
+    return totals, arrays
