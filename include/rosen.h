@@ -313,6 +313,23 @@ ROSEN_API size_t rosen_workspace_bytes(void);
 ROSEN_API int rosen_workspace_release(void);
 
 /*
+ * Test and tuning knobs (process-wide; value 0 restores the default). The library never reads the environment: these are
+ * the only way to change which kernel serves a chain length, so a stray variable cannot alter results at the 1e-12 level.
+ *   "lattice_hash_min_n"   2 .. 513   chain length from which rosen_lattice_generate uses the hash-map kernel
+ *   "realspace_cell_min_n" 2 .. 2049  same for rosen_realspace_generate and the cell-list kernel
+ *   "realspace_cand_cap"   33 .. 160  candidates a warp of the cell-list kernel buffers before a flush (33: every round)
+ *   "hash_blocks_per_sm"   1 .. 32    cap on resident blocks of the hash-map kernel (tuning)
+ *   "generations_left"     >= 0       not a knob but an action on the current device's long-chain workspace (there must be
+ *                                     one): every thread / warp of the next long-chain calls of the same layout wraps its
+ *                                     generation counter -- clears its table and restarts -- after `value` more chains.
+ *                                     Clears the tables (no old entry may carry a generation that is about to be used
+ *                                     again) and synchronises the device.
+ * Decisions (trajectory, m sequence, digest) never depend on a knob. Returns ROSEN_EINVAL for an unknown name or a value
+ * out of range.
+ */
+ROSEN_API int rosen_debug_set(const char* knob, int64_t value);
+
+/*
  * Number of kernel launches the last generate/dump call on this thread enqueued, and the name of
  * the main kernel variant it chose (static string). For bench.py's gpu_launches and profiles.
  */

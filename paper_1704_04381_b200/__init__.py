@@ -8,6 +8,6 @@ from .binding import (  # noqa: F401
     rosen_lattice_dump, rosen_lattice_generate, rosen_lattice_generate_async, rosen_lattice_generate_noalloc,
     ROSEN_NOALLOC_MAX_N, ROSEN_NOALLOC_MAX_CHAINS, ROSEN_NOALLOC_SCRATCH_BYTES, rosen_realspace_generate_async,
     SUMMARY_BYTES, summary_from_device, rosen_realspace_dump, rosen_realspace_generate, rosen_strerror,
-    rosen_summary_merge, rosen_fit_exponents, rosen_direction_eval, rosen_realspace_dump_probe, rosen_lattice_perm, rosen_lattice_generate_model, rosen_realspace_generate_model, rosen_version, rosen_workspace_bytes, rosen_workspace_release,
+    rosen_summary_merge, rosen_fit_exponents, rosen_direction_eval, rosen_realspace_dump_probe, rosen_lattice_perm, rosen_lattice_generate_model, rosen_realspace_generate_model, rosen_version, rosen_debug_set, rosen_workspace_bytes, rosen_workspace_release,
 )
 from . import workloads  # noqa: F401

@@ -102,6 +102,8 @@ def load_library() -> C.CDLL:
     L.rosen_workspace_bytes.restype = C.c_size_t
     L.rosen_workspace_release.argtypes = []
     L.rosen_workspace_release.restype = C.c_int
+    L.rosen_debug_set.argtypes = [C.c_char_p, C.c_int64]
+    L.rosen_debug_set.restype = C.c_int
     L.rosen_last_launch_count.argtypes = []
     L.rosen_last_launch_count.restype = i32
     for name in ("rosen_last_kernel_name", "rosen_last_error", "rosen_version"):
@@ -372,6 +374,11 @@ def rosen_workspace_bytes() -> int:
 
 def rosen_workspace_release() -> int:
     return int(load_library().rosen_workspace_release())
+
+
+def rosen_debug_set(knob: str, value: int) -> None:
+    """rosen_debug_set of include/rosen.h (test / tuning knobs; 0 = default)."""
+    _check(load_library().rosen_debug_set(knob.encode(), int(value)))
 
 
 def rosen_last_launch_count() -> int:

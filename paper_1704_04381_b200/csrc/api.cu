@@ -4,11 +4,13 @@
 #include "../../include/rosen.h"
 #include "common.cuh"
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <vector>
 
 namespace {
 
@@ -178,24 +180,26 @@ int stream_conf_out(Scratch* sc, cudaStream_t gen_stream, const void* conf_dev, 
     return ROSEN_OK;
 }
 
+// Test and tuning knobs, set through rosen_debug_set() (rosen.h) and never read from the environment: a stray variable in
+// a user's shell must not change which kernel runs. 0 = the library's default.
+std::atomic<int32_t> g_knob_hash_min_n{0}, g_knob_cell_min_n{0}, g_knob_cand_cap{0}, g_knob_hash_blocks_per_sm{0};
+
 // chain length from which the lattice call uses the hash-map kernel: measured crossover with the O(N^2) scan kernel
-// (2^24 chains: N = 128 scan 26.8 ms / hash 42.8 ms; N = 256 scan 152 ms / hash 84 ms). ROSEN_LATTICE_HASH_MIN_N overrides
-// it in 2 .. 513 (tests run either kernel over the other's range; results do not depend on the choice).
+// (2^24 chains: N = 128 scan 26.8 ms / hash 42.8 ms; N = 256 scan 152 ms / hash 84 ms). The knob lattice_hash_min_n overrides
+// it in 2 .. 513 (tests run either kernel over the other's range; decisions do not depend on the choice).
 int32_t hash_min_n()
 {
-    const char* e = std::getenv("ROSEN_LATTICE_HASH_MIN_N");
-    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_LATTICE_SCAN_MAX_N + 1) return (int32_t)v; }
-    return ROSEN_LATTICE_HASH_MIN_N;
+    const int32_t v = g_knob_hash_min_n.load();
+    return v ? v : ROSEN_LATTICE_HASH_MIN_N;
 }
 
 // same for the real-space call (cell-list kernel, realspace_long.cu): measured crossover with the shared-memory scan
-// kernel between N = 340 (k = 16) and N = 470 (k = 64); at N = 2048 the cell list is 10x faster. ROSEN_REALSPACE_CELL_MIN_N
-// overrides it in 2 .. 2049.
+// kernel between N = 340 (k = 16) and N = 470 (k = 64); at N = 2048 the cell list is 10x faster. Knob realspace_cell_min_n,
+// 2 .. 2049.
 int32_t cell_min_n()
 {
-    const char* e = std::getenv("ROSEN_REALSPACE_CELL_MIN_N");
-    if (e && *e) { const long v = std::strtol(e, nullptr, 10); if (v >= 2 && v <= ROSEN_REALSPACE_SCAN_MAX_N + 1) return (int32_t)v; }
-    return ROSEN_REALSPACE_CELL_MIN_N;
+    const int32_t v = g_knob_cell_min_n.load();
+    return v ? v : ROSEN_REALSPACE_CELL_MIN_N;
 }
 
 struct Sizes { size_t lnW, alive, m_seq, digest, conf, ree2, rg2; };
@@ -321,7 +325,7 @@ int lattice_impl(int32_t N, uint64_t n_chains, uint64_t seed, uint64_t chain_off
         hp.entries = rosen::hash_entries(N);
         const size_t table_bytes = (size_t)16 * hp.entries;               // 16-byte entries
         int max_threads = 0;
-        if (rosen::hash_max_threads(&max_threads) < 0) return fail_cuda(cudaGetLastError(), "device query");
+        if (rosen::hash_max_threads(&max_threads, g_knob_hash_blocks_per_sm.load()) < 0) return fail_cuda(cudaGetLastError(), "device query");
         uint64_t threads = (n_chains + 255) / 256 * 256;
         if (threads > (uint64_t)max_threads) threads = (uint64_t)max_threads;
         const uint64_t by_mem = kHashTableCap / table_bytes / 256 * 256;
@@ -405,10 +409,7 @@ int realspace_impl(int32_t N, uint64_t n_chains, int32_t k_trials, float bond_le
         lp.n_pad = ((uint32_t)N + 7u) & ~7u;
         lp.entries = rosen::hash_entries(N);
         lp.cand_cap = rosen::kRealLongCandCap;
-        if (const char* e = std::getenv("ROSEN_REALSPACE_CAND_CAP")) {   // test hook: force the flush path (results do not depend on it)
-            const long v = std::strtol(e, nullptr, 10);
-            if (v >= 33 && v <= (long)rosen::kRealLongCandCap) lp.cand_cap = (uint32_t)v;
-        }
+        if (const int32_t v = g_knob_cand_cap.load()) lp.cand_cap = (uint32_t)v;   // test knob: 33 forces the flush path (results do not depend on it)
         lp.warp_bytes = ((uint64_t)lp.n_pad * 16u + (uint64_t)lp.entries * 16u + 255u) & ~(uint64_t)255u;
         int max_warps = 0;
         if (rosen::real_long_max_warps(k_trials, &max_warps) < 0) return fail_cuda(cudaGetLastError(), "device query");
@@ -926,6 +927,51 @@ int rosen_workspace_release(void)
     cudaGetLastError();
     return ROSEN_OK;
 }
+int rosen_debug_set(const char* knob, int64_t value)
+{
+    g_err[0] = 0;
+    if (!knob) { std::snprintf(g_err, sizeof(g_err), "rosen_debug_set: knob is NULL"); return ROSEN_EINVAL; }
+    auto set = [&](std::atomic<int32_t>& k, int64_t lo, int64_t hi) -> int {
+        if (value != 0 && (value < lo || value > hi)) {
+            std::snprintf(g_err, sizeof(g_err), "rosen_debug_set(%s): %lld outside %lld .. %lld (0 = default)", knob, (long long)value, (long long)lo, (long long)hi);
+            return ROSEN_EINVAL;
+        }
+        k.store((int32_t)value);
+        return ROSEN_OK;
+    };
+    if (!std::strcmp(knob, "lattice_hash_min_n")) return set(g_knob_hash_min_n, 2, ROSEN_LATTICE_SCAN_MAX_N + 1);
+    if (!std::strcmp(knob, "realspace_cell_min_n")) return set(g_knob_cell_min_n, 2, ROSEN_REALSPACE_SCAN_MAX_N + 1);
+    if (!std::strcmp(knob, "realspace_cand_cap")) return set(g_knob_cand_cap, 33, (int64_t)rosen::kRealLongCandCap);
+    if (!std::strcmp(knob, "hash_blocks_per_sm")) return set(g_knob_hash_blocks_per_sm, 1, 32);
+    if (!std::strcmp(knob, "generations_left")) {
+        // every generation counter of the current device's long-chain workspace := (largest generation of the kernel the
+        // workspace was last laid out for) - value, so that each thread / warp clears its table and restarts at
+        // generation 1 after `value` more chains: the only way a test reaches that branch (2^25 / 2^19 chains per thread otherwise)
+        int dev = 0;
+        CK(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= kMaxDevices) return ROSEN_EINVAL;
+        Scratch& sc = g_scratch[dev];
+        std::lock_guard<std::mutex> call_lock(sc.call_mutex);
+        std::lock_guard<std::mutex> lock(g_mutex);
+        const uint64_t kind = sc.ws_layout >> 62;
+        if (!sc.hash_gen || (kind != 1 && kind != 2)) {
+            std::snprintf(g_err, sizeof(g_err), "rosen_debug_set(generations_left): no long-chain workspace on this device yet");
+            return ROSEN_EINVAL;
+        }
+        const uint32_t gen_max = kind == 1 ? rosen::lattice_hash_gen_max() : rosen::real_long_gen_max();
+        if (value < 0 || value > (int64_t)gen_max) { std::snprintf(g_err, sizeof(g_err), "rosen_debug_set(generations_left): 0 .. %u", gen_max); return ROSEN_EINVAL; }
+        CK(cudaDeviceSynchronize());
+        // the tables are cleared too: entries of earlier calls may carry the very generations the preset counters are about
+        // to run through again, which never happens when the counters only count up
+        CK(cudaMemset(sc.hash_tables, 0, sc.hash_tables_bytes));
+        const std::vector<uint32_t> host(kMaxGenSlots, gen_max - (uint32_t)value);
+        CK(cudaMemcpy(sc.hash_gen, host.data(), kMaxGenSlots * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        return ROSEN_OK;
+    }
+    std::snprintf(g_err, sizeof(g_err), "rosen_debug_set: unknown knob '%s'", knob);
+    return ROSEN_EINVAL;
+}
+
 int32_t rosen_last_launch_count(void) { return g_launches; }
 const char* rosen_last_kernel_name(void) { return g_kernel; }
 

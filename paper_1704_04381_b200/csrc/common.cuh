@@ -170,7 +170,8 @@ int launch_lattice(const LatticeParams& p, cudaStream_t stream, const char** ker
 // lattice_hash.cu: table geometry for chain length N, resident thread capacity of the device, launch (generation
 // kernel over n_threads = multiple of 256 threads, then the per-record first reduction pass).
 uint32_t hash_entries(int32_t N);
-int hash_max_threads(int* threads_out);
+int hash_max_threads(int* threads_out, int blocks_per_sm_cap);   // cap: 0 = none (tuning knob; results do not depend on it)
+uint32_t lattice_hash_gen_max();  // largest generation tag of a table entry (the counter wraps beyond it)
 int launch_lattice_hash(const HashParams& p, int n_threads, cudaStream_t stream, const char** kernel_name);
 // reduce_records_kernel of lattice_hash.cu: first reduction pass over per-chain records (+ optional per-chain outputs)
 // lmax != nullptr: first find L = max lnW (two launches), left in lmax[kMaxPartials]. Returns the launches made.
@@ -178,6 +179,7 @@ int launch_reduce_records(const ChainRecord* rec, uint64_t n_chains, uint32_t ch
                           double* lmax, const DevOutputs& out, Partial* partials, cudaStream_t stream);
 // realspace_long.cu: resident warp capacity, launch over n_warps (multiple of 8) warps + the record reduction
 int real_long_max_warps(int k, int* warps_out);
+uint32_t real_long_gen_max();
 int launch_realspace_long(const RealLongParams& p, int n_warps, cudaStream_t stream, const char** kernel_name);
 int launch_realspace(const RealParams& p, cudaStream_t stream, const char** kernel_name, int* grid_out);
 // realspace.cu: the D1 store phase alone over a resident synthetic chain (measurement entry rosen_realspace_dump_probe)

@@ -319,17 +319,16 @@ uint32_t hash_entries(int32_t N)
     return ((uint32_t)N + 8u) & ~7u;                   // a multiple of 8 (whole 128-byte lines) and >= N + 1 > cubes one chain can touch
 }
 
-int hash_max_threads(int* threads_out)
+uint32_t lattice_hash_gen_max() { return kGenMax; }
+
+int hash_max_threads(int* threads_out, int blocks_per_sm_cap)
 {
     int dev = 0, n_sm = 0, per_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
     // the traj variant has the larger register footprint: size the tables for the plain one, which every launch may use
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lattice_hash_kernel<false, false>, 256, 0) != cudaSuccess || per_sm < 1) return -3;
-    if (const char* e = std::getenv("ROSEN_HASH_BLOCKS_PER_SM")) {     // tuning knob (results do not depend on it)
-        const int v = std::atoi(e);
-        if (v >= 1 && v < per_sm) per_sm = v;
-    }
+    if (blocks_per_sm_cap >= 1 && blocks_per_sm_cap < per_sm) per_sm = blocks_per_sm_cap;
     *threads_out = n_sm * per_sm * 256;
     return 0;
 }

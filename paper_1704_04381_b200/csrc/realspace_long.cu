@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerBlock) realspace_long_kernel(con
         const uint32_t c_lo = (uint32_t)chain, c_hi = (uint32_t)(chain >> 32);
         if (++gen > kGenMax) {
             for (uint32_t i = lane; i < entries; i += 32) table[i] = make_ulonglong2(0ull, 0ull);
+            __syncwarp();                   // every lane's clears land before lane 0 enters the origin's cell below
             gen = 1u;
         }
         const uint64_t tag = (uint64_t)gen << kGenShift;
@@ -291,6 +292,8 @@ int launch_p(const RealLongParams& p, int n_warps, cudaStream_t stream)
 }
 
 }  // namespace
+
+uint32_t real_long_gen_max() { return kGenMax; }
 
 int real_long_max_warps(int k, int* warps_out)
 {

@@ -28,3 +28,13 @@ def read_golden(name):
 @pytest.fixture(scope="session")
 def golden():
     return read_golden
+
+
+@pytest.fixture(autouse=True)
+def _default_debug_knobs():
+    """rosen_debug_set knobs are process-wide: whatever a test set is back at its default for the next one, pass or fail."""
+    yield
+    from paper_1704_04381_b200 import binding
+    if binding._lib is not None:
+        for knob in ("lattice_hash_min_n", "realspace_cell_min_n", "realspace_cand_cap", "hash_blocks_per_sm"):
+            binding._lib.rosen_debug_set(knob.encode(), 0)

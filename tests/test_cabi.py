@@ -27,7 +27,7 @@ def declared_symbols():
 def test_every_declared_symbol_is_exported(R):
     from paper_1704_04381_b200 import binding
     names = declared_symbols()
-    assert len(names) == 21 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
+    assert len(names) == 22 and "rosen_lattice_generate" in names and "rosen_realspace_dump" in names
     lib = ctypes.CDLL(binding.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), n
@@ -59,6 +59,22 @@ def test_host_only_entry_points(R):
     assert math.isclose(m["ln_mean_W"], 3.0 + math.log((4.0 * f + 12.0) / 40), rel_tol=1e-15)
     with pytest.raises(R.RosenError):
         R.rosen_summary_merge([a, dict(b, ln_shift=float("inf"))])
+
+
+def test_debug_knobs_validate_and_ignore_the_environment(R, monkeypatch):
+    """The knobs exist only behind rosen_debug_set; names and ranges are checked; nothing in the library reads getenv."""
+    for knob, good, bad in [("lattice_hash_min_n", 2, 514), ("realspace_cell_min_n", 2049, 1), ("realspace_cand_cap", 33, 32),
+                            ("hash_blocks_per_sm", 1, 33)]:
+        R.rosen_debug_set(knob, good)
+        with pytest.raises(R.RosenError):
+            R.rosen_debug_set(knob, bad)
+        R.rosen_debug_set(knob, 0)
+    with pytest.raises(R.RosenError):
+        R.rosen_debug_set("no_such_knob", 1)
+    for src in os.listdir(os.path.join(ROOT, "paper_1704_04381_b200", "csrc")):
+        if not src.endswith((".cu", ".cuh")):
+            continue
+        assert "getenv" not in open(os.path.join(ROOT, "paper_1704_04381_b200", "csrc", src)).read(), src
 
 
 def test_no_cpu_fallback(R):

@@ -90,16 +90,16 @@ def test_long_chains_hash_kernel(R, N, n_chains, seed, offset):
 
 
 def test_scan_kernel_over_its_whole_range(R, monkeypatch):
-    """By default N >= ROSEN_LATTICE_HASH_MIN_N = 193 takes the hash-map kernel; ROSEN_LATTICE_HASH_MIN_N=513 keeps the
+    """By default N >= ROSEN_LATTICE_HASH_MIN_N = 193 takes the hash-map kernel; the knob lattice_hash_min_n = 513 keeps the
     scan kernel up to its limit N = 512 so that its wide variant stays covered against the oracle."""
-    monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "513")
+    R.rosen_debug_set("lattice_hash_min_n", 513)
     for N, n, seed in [(193, 800, 12), (256, 1200, 11), (300, 300, 13), (512, 200, 14)]:
         s, t = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
         assert "lattice_dp_kernel<wide" in R.rosen_last_kernel_name()
         o = oracle.lattice_generate(N, n, seed)
         compare_per_chain(t, o, N)
         compare_summary(s, o.summary)
-    monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N")
+    R.rosen_debug_set("lattice_hash_min_n", 0)
     R.rosen_lattice_generate(192, 100, 1)
     assert "lattice_dp_kernel" in R.rosen_last_kernel_name()
     R.rosen_lattice_generate(193, 100, 1)
@@ -107,15 +107,15 @@ def test_scan_kernel_over_its_whole_range(R, monkeypatch):
 
 
 def test_hash_kernel_equals_scan_kernel_on_short_chains(R, monkeypatch):
-    """ROSEN_LATTICE_HASH_MIN_N routes short chains through the hash kernel: it must reproduce the scan kernel
+    """The knob lattice_hash_min_n = 2 routes short chains through the hash kernel: it must reproduce the scan kernel
     (and with it the oracle and its enumeration pins) bit for bit, per chain and in the ensemble sums, with
     many chains per lane (table generations) and more chains than resident threads."""
     import torch
     for N, n, seed in [(16, 1 << 16, 1), (64, 400000, 7), (200, 30011, 3)]:
-        monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "513")
+        R.rosen_debug_set("lattice_hash_min_n", 513)
         s_scan, t_scan = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
         assert "lattice_dp_kernel" in R.rosen_last_kernel_name()
-        monkeypatch.setenv("ROSEN_LATTICE_HASH_MIN_N", "2")
+        R.rosen_debug_set("lattice_hash_min_n", 2)
         s_hash, t_hash = R.rosen_lattice_generate(N, n, seed, outputs=ALL)
         assert "lattice_hash_kernel" in R.rosen_last_kernel_name()
         for k in ALL:
@@ -128,7 +128,7 @@ def test_hash_kernel_equals_scan_kernel_on_short_chains(R, monkeypatch):
             assert s_scan[k] == s_hash[k], k
         for k in ("sum_w", "sum_w_ree2", "sum_w_rg2", "sum_w2", "mean_ree2", "mean_rg2", "ln_mean_W"):
             assert math.isclose(s_scan[k], s_hash[k], rel_tol=REL), k
-    monkeypatch.delenv("ROSEN_LATTICE_HASH_MIN_N", raising=False)
+    R.rosen_debug_set("lattice_hash_min_n", 0)
     assert R.rosen_workspace_bytes() > (1 << 20)
     assert R.rosen_workspace_release() == R.ROSEN_OK
 
@@ -352,3 +352,28 @@ def test_workspace_release_while_other_threads_call(R):
     assert R.rosen_workspace_release() == R.ROSEN_OK
     s2, t2 = R.rosen_lattice_generate(*jobs[1], outputs=("digest", "lnW"))       # everything released is made again
     assert s2 == want[1][0] and torch.equal(t2["digest"], want[1][1]["digest"])
+
+
+def test_generation_counter_wrap_of_the_hash_kernel(R):
+    """Every thread of the hash-map kernel tags its table entries with a generation counter that persists across calls; when
+    it passes its largest value the thread clears its table and restarts at 1 (lattice_hash.cu). Reaching that naturally takes
+    2^25 chains per thread: rosen_debug_set("generations_left", g) presets the counters so that it happens g chains from now,
+    in the middle of a call whose tables are full of entries of the generations just below the limit."""
+    import torch
+    R.rosen_debug_set("hash_blocks_per_sm", 1)       # 148 x 256 resident threads: every thread grows ~5 chains of the call,
+    N, n, seed = 600, 200000, 41                     # so the wrap falls between chains, on a table full of this call's entries
+    s0, t0 = R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW", "alive"))
+    assert "lattice_hash_kernel" in R.rosen_last_kernel_name()
+    o = oracle.lattice_generate(N, 3000, seed, outputs=("digest",))
+    assert np.array_equal(t0["digest"][:3000].cpu().numpy().view(np.uint64), o.digest)
+    for left in (0, 1, 2, 4):
+        R.rosen_debug_set("generations_left", left)
+        s1, t1 = R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW", "alive"))
+        assert s1 == s0, left
+        for k in t0:
+            assert torch.equal(t0[k], t1[k]), (left, k)
+    s2, _ = R.rosen_lattice_generate(N, n, seed, outputs=("digest", "lnW", "alive"))      # and the calls after the wrap
+    assert s2 == s0
+    R.rosen_workspace_release()
+    with pytest.raises(R.RosenError):
+        R.rosen_debug_set("generations_left", 1)     # no workspace: refused, nothing to preset

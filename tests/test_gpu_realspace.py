@@ -79,13 +79,13 @@ def test_shapes_ragged_and_edges(R, N, n, k, b, sigma, seed, offset):
 
 
 def test_scan_kernel_over_its_whole_range(R, monkeypatch):
-    """By default N >= ROSEN_REALSPACE_CELL_MIN_N = 400 takes the cell-list kernel; ROSEN_REALSPACE_CELL_MIN_N=2049 keeps
+    """By default N >= ROSEN_REALSPACE_CELL_MIN_N = 400 takes the cell-list kernel; the knob realspace_cell_min_n = 2049 keeps
     the shared-memory scan kernel up to its limit so that its long-chain variants stay covered against the oracle."""
-    monkeypatch.setenv("ROSEN_REALSPACE_CELL_MIN_N", "2049")
+    R.rosen_debug_set("realspace_cell_min_n", 2049)
     for args in [(400, 20, 16, 1.0, 1.0, 13, 0), (1024, 6, 4, 1.0, 0.6, 15, 0), (1024, 3, 2, 0.5, 0.0, 15, 2), (2048, 3, 3, 1.0, 0.5, 16, 1)]:
         check(R, *args)
         assert R.rosen_last_kernel_name().startswith("realspace_kernel")
-    monkeypatch.delenv("ROSEN_REALSPACE_CELL_MIN_N")
+    R.rosen_debug_set("realspace_cell_min_n", 0)
     R.rosen_realspace_generate(399, 10, 4, 1.0, 0.5, 1)
     assert R.rosen_last_kernel_name().startswith("realspace_kernel")
     R.rosen_realspace_generate(400, 10, 4, 1.0, 0.5, 1)
@@ -113,14 +113,34 @@ def test_cell_list_workspace_reuse_across_neighbouring_lengths(R):
         assert "realspace_long_kernel" in R.rosen_last_kernel_name()
 
 
+def test_generation_counter_wrap_of_the_cell_list_kernel(R):
+    """As the lattice test of the same name: every warp of the cell-list kernel keeps a generation counter across calls and
+    clears its cell table when it wraps (2^19 chains per warp: reachable by a long-lived process). generations_left presets
+    the counters so that the wrap falls inside a call, between chains whose entries sit just below the limit."""
+    R.rosen_debug_set("realspace_cell_min_n", 2)
+    N, n, k, b, sigma, seed = 48, 60000, 8, 1.0, 0.9, 51       # more chains than resident warps: several chains per warp
+    s0, t0 = R.rosen_realspace_generate(N, n, k, b, sigma, seed, outputs=("digest", "lnW"))
+    assert "realspace_long_kernel" in R.rosen_last_kernel_name()
+    o = oracle.realspace_generate(N, 4000, k, b, sigma, seed, outputs=("digest",))
+    assert np.array_equal(t0["digest"][:4000].cpu().numpy().view(np.uint64), o.digest)
+    import torch
+    for left in (0, 1, 3):
+        R.rosen_debug_set("generations_left", left)
+        s1, t1 = R.rosen_realspace_generate(N, n, k, b, sigma, seed, outputs=("digest", "lnW"))
+        assert s1 == s0, left
+        assert torch.equal(t0["digest"], t1["digest"]) and torch.equal(t0["lnW"], t1["lnW"]), left
+    s2, _ = R.rosen_realspace_generate(N, n, k, b, sigma, seed, outputs=("digest", "lnW"))
+    assert s2 == s0
+
+
 @pytest.mark.parametrize("cap", [None, "33"])
 def test_cell_list_kernel_on_short_chains(R, monkeypatch, cap):
-    """ROSEN_REALSPACE_CELL_MIN_N routes short chains through the cell-list kernel, where the oracle's full scan is
-    cheap enough for thousands of chains and every k variant; ROSEN_REALSPACE_CAND_CAP=33 makes the candidate buffer
+    """The knob realspace_cell_min_n = 2 routes short chains through the cell-list kernel, where the oracle's full scan is
+    cheap enough for thousands of chains and every k variant; realspace_cand_cap = 33 makes the candidate buffer
     flush after every round, the path dense configurations take."""
-    monkeypatch.setenv("ROSEN_REALSPACE_CELL_MIN_N", "2")
+    R.rosen_debug_set("realspace_cell_min_n", 2)
     if cap:
-        monkeypatch.setenv("ROSEN_REALSPACE_CAND_CAP", cap)
+        R.rosen_debug_set("realspace_cand_cap", int(cap))
     for N, n, k, b, sigma, seed in [(2, 50, 5, 1.0, 1.0, 1), (3, 3000, 16, 1.0, 1.0, 3), (16, 2001, 7, 0.7, 1.0, 6),
                                     (64, 4000, 16, 1.0, 1.0, 3), (40, 500, 33, 1.0, 0.0, 8), (25, 300, 65, 1.0, 0.8, 11),
                                     (18, 200, 129, 1.0, 1.0, 12), (12, 100, 255, 1.0, 1.0, 12), (256, 300, 64, 1.0, 0.8, 13),
@@ -129,7 +149,7 @@ def test_cell_list_kernel_on_short_chains(R, monkeypatch, cap):
         assert "realspace_long_kernel" in R.rosen_last_kernel_name()
     s0, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3)
     s1, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3, outputs=ALL)
-    monkeypatch.delenv("ROSEN_REALSPACE_CELL_MIN_N")
+    R.rosen_debug_set("realspace_cell_min_n", 0)
     s2, _ = R.rosen_realspace_generate(64, 30011, 16, 1.0, 1.0, 3)
     assert "realspace_kernel" in R.rosen_last_kernel_name()
     for key in s0:
