@@ -255,6 +255,92 @@ def time_oracle_all_cores(w: workloads.Workload, per_thread: int, threads: int):
     return per_thread * threads, time.perf_counter() - t0
 
 
+def alg_warp_inst(w: workloads.Workload, steps_attempted: float):
+    """Algorithmic warp-instructions of one launch under the models of DESIGN.md 6, and the model in words (the same
+    numbers run_product uses for the headline workload)."""
+    if w.kind == "lattice" and w.N >= 193:
+        return HASH_INSTR_PER_STEP * steps_attempted / 32.0, f"{HASH_INSTR_PER_STEP} thread-instr per attempted step (hash-map kernel)"
+    if w.kind == "realspace" and w.N >= 400:
+        per = w.k_trials * (80.0 + 7.0 * 3.2) + 27 * 14.0 + 40 * 10.0 + 50.0
+        return per * steps_attempted / 32.0, f"{per:.1f} thread-instr per attempted step (cell-list kernel)"
+    per = algorithmic_thread_instr(w)
+    return per * w.n_chains / 32.0, f"{per:.0f} thread-instr per chain"
+
+
+def oracle_digests(w: workloads.Workload, n: int):
+    """Per-chain digests of chain ids [0, n) from the oracle on all host cores (disjoint ranges, results concatenated)."""
+    import numpy as np
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    threads = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    parts = max(1, min(n, threads * 4))
+    bounds = [n * i // parts for i in range(parts + 1)]
+
+    def one(i):
+        return oracle.realspace_generate(w.N, bounds[i + 1] - bounds[i], w.k_trials, w.bond_len, w.sigma, w.seed,
+                                         chain_offset=bounds[i], outputs=("digest",)).digest
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        return np.concatenate(list(ex.map(one, range(parts))))
+
+
+def measure_brief(R, torch, w: workloads.Workload, stream, timed, peak_winst: float, hbm_gbs: float, steps: int, flip_sample: int):
+    """One entry of the `configs` block: workload w timed in this process with the method of the headline leg (CUDA events
+    on the launching stream, L2 flushed between steps, 3 warm-up steps), generation kernel alone, the synchronous
+    host-buffer call end to end, the roofline fraction under the DESIGN.md 6 model, and for real space the flip fraction
+    of the first `flip_sample` chains against the oracle and (dump workload) the store-phase bandwidth."""
+    enqueue, sync_call, d2h_bytes = make_calls(R, torch, w, 0, stream)
+    summary_dev = torch.zeros(R.SUMMARY_BYTES, dtype=torch.uint8, device="cuda")
+    timed(lambda: enqueue(summary_dev), 3)
+    launches, kernel_name = R.rosen_last_launch_count(), R.rosen_last_kernel_name()
+    ms = timed(lambda: enqueue(summary_dev), steps)
+    summary = R.summary_from_device(summary_dev)
+    timed(lambda: enqueue(None), 1)
+    kms = timed(lambda: enqueue(None), max(3, steps // 2))
+    kernel_ms = sum(kms) / len(kms)
+    sync_call()
+    e0 = time.perf_counter()
+    for _ in range(3):
+        sync_call()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - e0) / 3 * 1e3
+    ms_per_step = sum(ms) / len(ms)
+    alg, model = alg_warp_inst(w, summary["n_steps_attempted"])
+    entry = {
+        "N": w.N, "n_chains": w.n_chains, "seed": w.seed, "k_trials": w.k_trials, "steps": steps, "warmup": 3,
+        "ms_per_step": ms_per_step, "chains_per_s": w.n_chains / (ms_per_step * 1e-3),
+        "monomer_steps_per_s": summary["n_steps_attempted"] / (ms_per_step * 1e-3),
+        "kernel": kernel_name, "kernel_ms": kernel_ms, "gpu_launches_per_step": launches,
+        "roofline": {"bound": "alu", "frac": alg / (kernel_ms * 1e-3) / peak_winst, "achieved": alg / (kernel_ms * 1e-3) / 1e9,
+                     "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s", "model": model},
+        "e2e_ms_per_step": e2e_ms, "e2e_chains_per_s": w.n_chains / (e2e_ms * 1e-3), "d2h_bytes_per_step": d2h_bytes,
+        "attrition": summary["attrition"], "mean_ree2": summary["mean_ree2"],
+    }
+    if w.kind == "realspace" and flip_sample:
+        import numpy as np
+        n = min(flip_sample, w.n_chains)
+        _, tg = R.rosen_realspace_generate(w.N, n, w.k_trials, w.bond_len, w.sigma, w.seed, outputs=("digest",))
+        ref = oracle_digests(w, n)
+        entry["flip_fraction"] = {"value": float((tg["digest"].cpu().numpy().view(np.uint64) != ref).mean()), "chains": n, "bar": 1e-4}
+    if w.dump and w.kind == "realspace":
+        def gen_only():
+            R.rosen_realspace_generate_async(w.N, w.n_chains, w.k_trials, w.bond_len, w.sigma, w.seed, 0, outputs=None,
+                                             summary_device=None, stream=stream)
+        conf = torch.empty((w.n_chains, w.N, 3), dtype=torch.float32, device="cuda")
+        lnw = torch.empty((w.n_chains,), dtype=torch.float64, device="cuda")
+        timed(gen_only, 1)
+        t_gen, t_all = min(timed(gen_only, 3)), min(kms)
+        timed(lambda: R.rosen_realspace_dump_probe(w.N, w.n_chains, conf, lnw, stream=stream), 2)
+        t_probe = min(timed(lambda: R.rosen_realspace_dump_probe(w.N, w.n_chains, conf, lnw, stream=stream), 5))
+        nbytes = w.n_chains * (12 * w.N + 8)
+        diff = t_all - t_gen
+        entry["dump_path"] = {"bytes_per_step": nbytes, "with_dump_ms": t_all, "generation_only_ms": t_gen,
+                              "in_situ_store_GBps": nbytes / (diff * 1e-3) / 1e9 if diff > 0.01 * t_all else None,
+                              "isolated_store_ms": t_probe, "isolated_store_GBps": nbytes / (t_probe * 1e-3) / 1e9,
+                              "peak_GBps": hbm_gbs, "isolated_store_frac": nbytes / (t_probe * 1e-3) / 1e9 / hbm_gbs}
+        del conf, lnw
+    return entry
+
+
 def run_reference(args, w, rank):
     """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
     if rank != 0:
@@ -488,6 +574,20 @@ def run_product(args, w, rank, world, local_rank):
                                "sample": f"{cores} threads x {per} chains (disjoint chain-id ranges of {w.name}), {dta:.1f} s",
                                "single_thread": {"value": m / dt, "cores": 1,
                                                  "sample": f"chain ids [0, {m}) of {w.name}, {dt:.1f} s"}}
+    if world == 1 and w.name == DEFAULT_WORKLOAD and not args.no_configs:
+        # every other BASELINE configuration in the same process, after the headline leg, so
+        # that the one line the driver records carries a number for each: configs 1, 3, 5 and the six points of config 4
+        sampler2 = ClockSampler(local_rank); sampler2.start()
+        c0 = time.perf_counter()
+        block = {}
+        for cw in (workloads.CONFIG_1, workloads.CONFIG_3, workloads.CONFIG_5, *workloads.CONFIG_4):
+            block[cw.name] = measure_brief(R, torch, cw, stream, timed, peak_winst, float(peaks.get("hbm_gbs", 6650.0)),
+                                           steps=max(5, min(steps, 10)), flip_sample=0 if args.no_cpu_baseline else 1 << 13)
+            torch.cuda.empty_cache()
+        c1 = time.perf_counter()
+        out["configs"] = block
+        out["configs_clocks"] = sampler2.stop(c0, c1)
+        out["configs_wall_s"] = c1 - c0
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
@@ -597,6 +697,7 @@ def main():
     ap.add_argument("--impl", default="product", choices=("product", "reference"))
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="default workload only: skip the block that times every other BASELINE config")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE config 4 (length sweep) instead")
     ap.add_argument("--paper-tables", action="store_true", help="10^6 chains at every length of the paper's Tables 1-2 instead")
     args = ap.parse_args()
