@@ -53,7 +53,9 @@ __device__ __forceinline__ uint64_t scaled_target(uint32_t u, uint64_t W)
     return (W >> 32) * (uint64_t)u + (((W & 0xFFFFFFFFull) * (uint64_t)u) >> 32);
 }
 
-template <int Z, bool TRAJ>
+// CONTACTS = false: every factor Q[c] is the same number (beta eps = 0: q = 1), so the contact counts cannot influence a
+// weight or a choice and are not formed; the decisions are the same bits either way (the host picks the variant from Q).
+template <int Z, bool TRAJ, bool CONTACTS>
 __global__ void __launch_bounds__(256) lattice_model_kernel(const ModelParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -118,7 +120,7 @@ __global__ void __launch_bounds__(256) lattice_model_kernel(const ModelParams p)
                 trial_offset<Z>(d, ex, ey, ez);
                 const int site = 62 + ex + 5 * ey + 25 * ez;                 // compile-time after unrolling
                 const bool occ = site < 64 ? ((mlo >> site) & 1ull) != 0ull : ((mhi >> (site - 64)) & 1ull) != 0ull;
-                const int c = __popcll(mlo & nb[2 * d]) + __popcll(mhi & nb[2 * d + 1]);
+                const int c = CONTACTS ? __popcll(mlo & nb[2 * d]) + __popcll(mhi & nb[2 * d + 1]) : 0;
                 wq[d] = occ ? 0ull : Qs[c];
                 W += wq[d]; m += occ ? 0u : 1u;
             }
@@ -164,8 +166,8 @@ __global__ void __launch_bounds__(256) lattice_model_kernel(const ModelParams p)
     }
 }
 
-template <int Z, bool TRAJ>
-int launch_variant(const ModelParams& p, cudaStream_t stream)
+template <int Z, bool TRAJ, bool CONTACTS>
+int launch_variant_c(const ModelParams& p, cudaStream_t stream)
 {
     int dev = 0, n_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -3;
@@ -174,13 +176,21 @@ int launch_variant(const ModelParams& p, cudaStream_t stream)
     int threads = 256;
     while (threads > 32 && fixed + (size_t)p.N * 4 * threads > (size_t)(72 * 1024)) threads >>= 1;
     const size_t smem = fixed + (size_t)p.N * 4 * threads;
-    auto kern = lattice_model_kernel<Z, TRAJ>;
+    auto kern = lattice_model_kernel<Z, TRAJ, CONTACTS>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -3;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) return -3;
     const uint64_t want = (p.n_chains + threads - 1) / threads, cap = (uint64_t)n_sm * per_sm;
     kern<<<(int)(want < cap ? want : cap), threads, smem, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? 1 : -3;
+}
+
+template <int Z, bool TRAJ>
+int launch_variant(const ModelParams& p, cudaStream_t stream)
+{
+    bool flat = true;                   // all factors equal (q = 1): contact counts are irrelevant
+    for (int c = 1; c < 32; ++c) flat = flat && p.Q[c] == p.Q[0];
+    return flat ? launch_variant_c<Z, TRAJ, false>(p, stream) : launch_variant_c<Z, TRAJ, true>(p, stream);
 }
 
 }  // namespace
