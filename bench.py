@@ -69,6 +69,8 @@ PROFILE_OF = {   # committed ncu summary (profiles/) of the dominant kernel of e
     "lattice_long_N1024_2p20": "r02_lattice_long_N1024.md", "lattice_long_N2048_2p19": "r02_lattice_long_N2048.md",
     "lattice_long_N10000_2p17": "r02_lattice_long_N10000.md", "realspace_long_N4096_k16_2p16": "r02_realspace_long_N4096.md",
     "realspace_long_N10000_k64_2p14": "r02_realspace_long_N10000.md",
+    "lattice_z6_contact0.3_N64_2p20": "r03_lattice_model_z6.md", "lattice_z26_N64_2p20": "r03_lattice_model_z26.md",
+    "realspace_well1.5_0.4_N64_k16_2p20": "r03_realspace_well.md", "lattice_perm_N256_2p20": "r03_lattice_perm.md",
 }
 
 
@@ -255,9 +257,35 @@ def time_oracle_all_cores(w: workloads.Workload, per_thread: int, threads: int):
     return per_thread * threads, time.perf_counter() - t0
 
 
+def model_thread_instr(w: workloads.Workload):
+    """(thread-instructions, "per chain" | "per attempted step") the METHOD needs for a model / PERM workload (DESIGN.md 6,
+    round 3): the base models with the terms these variants add.
+      lattice model   per chain: the box scan 8 per earlier monomer (3 coordinate range tests, map bit) over sum_s (s - 1)
+                      monomers; per step z trials x (occupancy 2 + weight / count / cumulative selection 5, + 4 for the
+                      contact popcount when beta eps > 0) + a quarter Philox block 17.5 + 30 (log, place, sums, digest)
+      square well     the config-3 model with 8 instead of 7 per pair test (second compare), 3 per trial for the
+                      fixed-point weight and its prefix sum, and 3.2 x ((b + lambda sigma) / (b + sigma))^3 candidates per
+                      trial (the candidate sphere reaches to the well's edge)
+      PERM            per node: 6 per site test over the (n - 2) / 2 monomers of the right parity, n ~ N / 2 on average over
+                      the nodes of a tour (approximation: the length distribution of nodes is flat to within the
+                      enrichment / pruning balance), + one Philox block 70 + 30 (count, choose, place, thresholds, stack)"""
+    N, k = w.N, w.k_trials
+    if w.perm is not None:
+        return 6.0 * (N / 2.0 - 2.0) / 2.0 + 70.0 + 30.0, "per attempted step"
+    if w.kind == "lattice":
+        per_trial = 7.0 + (4.0 if (w.beta_eps or 0.0) > 0.0 else 0.0)
+        return 8.0 * (N - 1) * (N - 2) / 2.0 + (N - 1) * (w.z * per_trial + 17.5 + 30.0), "per chain"
+    # candidates per trial grow with the volume of the candidate sphere: radius b + lambda sigma instead of b + sigma
+    cand = 3.2 * ((w.bond_len + w.lam * w.sigma) / (w.bond_len + w.sigma)) ** 3
+    return 7.0 * (N - 1) * (N - 2) / 2.0 + (N - 1) * (8.0 * cand * k + 35.0 * k + 45.0 * k + 3.0 * k + 30.0), "per chain"
+
+
 def alg_warp_inst(w: workloads.Workload, steps_attempted: float):
     """Algorithmic warp-instructions of one launch under the models of DESIGN.md 6, and the model in words (the same
     numbers run_product uses for the headline workload)."""
+    if w.perm is not None or w.beta_eps is not None:
+        per, unit = model_thread_instr(w)
+        return per * (steps_attempted if unit == "per attempted step" else w.n_chains) / 32.0, f"{per:.1f} thread-instr {unit}"
     if w.kind == "lattice" and w.N >= 193:
         return HASH_INSTR_PER_STEP * steps_attempted / 32.0, f"{HASH_INSTR_PER_STEP} thread-instr per attempted step (hash-map kernel)"
     if w.kind == "realspace" and w.N >= 400:
@@ -519,9 +547,12 @@ def run_product(args, w, rank, world, local_rank):
     if clocks.get("sm_mhz"):
         roofline["frac_at_measured_clock"] = achieved / (n_sm * 4 * clocks["sm_mhz"] * 1e6)
     if extra:
-        roofline = {"bound": "alu", "achieved": None, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s", "frac": None, "traffic": None,
-                    "kernel": kernel_name, "kernel_ms": kernel_ms,
-                    "note": "model / PERM workload (SURVEY.md 8(f) rows 4, 2): timed, no algorithmic-work model stated"}
+        alg_x, model_x = alg_warp_inst(w, steps_attempted / world)
+        ach_x = alg_x / (kernel_ms * 1e-3)
+        roofline = {"bound": "alu", "achieved": ach_x / 1e9, "peak": peak_winst / 1e9, "unit": "Gwarp-inst/s", "frac": ach_x / peak_winst,
+                    "traffic": prof.get("traffic"), "kernel": kernel_name, "kernel_ms": kernel_ms, "model": model_x,
+                    "peak_source": f"{n_sm} SMs x 4 schedulers x sm_max_mhz ({peaks_src} MEASURED_PEAKS.json)",
+                    "note": "model / PERM workload (SURVEY.md 8(f) rows 4, 2): kernel_ms covers the generation kernel + record reduction"}
     if w.kind == "lattice" and w.N < 193 and not extra:
         # SURVEY.md 8(d) wrote "930 x ~5" per site test where DESIGN.md 6 counts the 6 equality tests of the method: both
         survey = 5.0 * lattice_site_tests(w.N) + 70.0 * ((w.N + 3) // 4) + 20.0 * (w.N - 1)
