@@ -516,7 +516,7 @@ def run_product(args, w, rank, world, local_rank):
     alg_winst = algorithmic_thread_instr(w) * w.n_chains / 32.0
     achieved = alg_winst / (kernel_ms * 1e-3)
     if w.kind == "lattice" and w.N >= 193 and not extra:
-        # hash-map kernel (DESIGN.md 5.5 / 6): ncu shows it issue-bound (60.5 % issue-active, 28 % of DRAM peak), so the
+        # hash-map kernel (DESIGN.md 5.5 / 6): ncu shows it issue-bound (67 % issue-active, 11 % of DRAM peak), so the
         # roofline is the issue peak; algorithmic work per ATTEMPTED step (not per nominal step: most long chains die
         # early): 3 cube look-ups (hash 8 + compare 6 each), 6 occupancy bits (4 each), count/choose 15, insert 10,
         # observables 12, weight 3, a quarter Philox block 17.5 = 123.5 thread-instructions
